@@ -1,0 +1,455 @@
+"""Pins for the CPU oracle: the oracle is checked against things OTHER than itself --
+library routines (transformers' Qwen3 RoPE, torch SDPA, torch bf16 casts), closed forms, brute force, values the
+paper prints (tests/golden/paper_constants.txt) and invariants the method must have.  No GPU needed.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import hga_workloads as W
+import oracle
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")
+
+
+def golden():
+    vals = {}
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.split("#", 1)[0].strip()
+            if "=" in line:
+                k, v = line.split("=")
+                vals[k.strip()] = float(v)
+    return vals
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# Independent helpers (numpy / torch; none of this is shared with oracle/ or the CUDA path)
+# ----------------------------------------------------------------------------------------------------------------
+def rope_complex(x, pos, base):
+    """RoPE as a complex rotation: (x[i] + 1j*x[i+D/2]) * exp(1j*p*theta_i), fp64."""
+    x = np.asarray(x, dtype=np.float64)
+    D = x.shape[-1]
+    h = D // 2
+    theta = 1.0 / np.power(float(base), np.arange(h, dtype=np.float64) * 2.0 / D)
+    z = (x[..., :h] + 1j * x[..., h:]) * np.exp(1j * np.asarray(pos, dtype=np.float64)[..., None] * theta)
+    return np.concatenate([z.real, z.imag], axis=-1)
+
+
+def sdpa_causal(q, k, v):
+    """torch's scaled_dot_product_attention, causal, fp64 -- the paper's dense baseline."""
+    q, k, v = (torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)) for a in (q, k, v))
+    return torch.nn.functional.scaled_dot_product_attention(q[None], k[None].expand(1, q.shape[0], -1, -1),
+                                                            v[None].expand(1, q.shape[0], -1, -1),
+                                                            is_causal=True)[0].numpy()
+
+
+def nearest_bf16(x):
+    """Nearest bf16 to each fp64 value by brute force over the three neighbouring bf16 bit patterns
+    (ties -> even mantissa).  Independent of the oracle's frexp-based rounding."""
+    x = np.asarray(x, dtype=np.float64)
+    c = torch.from_numpy(x.astype(np.float32)).to(torch.bfloat16)
+    bits = c.view(torch.int16).to(torch.int32)
+    best, best_err, best_odd = None, None, None
+    for d in (-1, 0, 1):
+        b = (bits + d).to(torch.int16)
+        cand = b.view(torch.bfloat16).to(torch.float64).numpy()
+        err = np.abs(cand - x)
+        odd = (b.to(torch.int32) & 1).numpy()
+        if best is None:
+            best, best_err, best_odd = cand.copy(), err, odd
+        else:
+            take = (err < best_err) | ((err == best_err) & (odd < best_odd))
+            best = np.where(take, cand, best)
+            best_odd = np.where(take, odd, best_odd)
+            best_err = np.where(take, err, best_err)
+    return best
+
+
+def small_problem(seed=0, G=2, N=512, D=32, base=1.0e4, clustered=False):
+    w = W.Workload("t", 1, N, G, 1, D, "f32", base, topk_chunks=3, topk_groups=5,
+                   dist="clustered" if clustered else "iid", n_clusters=4)
+    q, k, v = W.generate(w, seed)
+    return w, q[0], k[0, 0], v[0, 0]
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# O1 RoPE
+# ----------------------------------------------------------------------------------------------------------------
+def test_rope_matches_transformers_qwen3():
+    """R6 convention = the Qwen3 family's: compare with transformers' own rotary code."""
+    from transformers import Qwen3Config
+    from transformers.models.qwen3.modeling_qwen3 import Qwen3RotaryEmbedding, apply_rotary_pos_emb
+
+    for D, base in ((64, 1.0e4), (128, 1.0e6)):
+        cfg = Qwen3Config(hidden_size=256, num_attention_heads=4, num_key_value_heads=1, head_dim=D,
+                          max_position_embeddings=4096, rope_theta=base)
+        if getattr(cfg, "rope_parameters", None) is not None:
+            cfg.rope_parameters["rope_theta"] = base
+        emb = Qwen3RotaryEmbedding(cfg)
+        x = torch.randn(1, 2, 48, D, dtype=torch.float64, generator=torch.Generator().manual_seed(1))
+        pos = torch.arange(5, 53)[None]
+        cos, sin = emb(x, pos)
+        ref, _ = apply_rotary_pos_emb(x, x, cos, sin)
+        got = oracle.rope(x[0].numpy().astype(np.float32), 5, base)
+        # transformers builds cos/sin in fp32 -> ~1e-6 agreement at these small positions
+        assert np.abs(got - ref[0].numpy()).max() < 2e-5
+
+
+def test_rope_complex_form_and_invariants():
+    rng = np.random.default_rng(0)
+    x = rng.standard_normal((3, 40, 64)).astype(np.float32)
+    got = oracle.rope(x, 1000, 1.0e4)
+    ref = rope_complex(x, np.arange(1000, 1040)[None, :].repeat(3, 0), 1.0e4)
+    assert np.abs(got - ref).max() < 1e-12
+    # norm preserving, identity at position 0
+    assert np.allclose(np.linalg.norm(got, axis=-1), np.linalg.norm(x.astype(np.float64), axis=-1), rtol=1e-13)
+    assert np.array_equal(oracle.rope(x[:, :1], 0, 1.0e4), x[:, :1].astype(np.float64))
+    # relative-position property: <R(p)q, R(t)k> depends on p - t only
+    q = rng.standard_normal((1, 64)).astype(np.float32)
+    k = rng.standard_normal((1, 64)).astype(np.float32)
+    a = oracle.rope(q, 900, 1.0e4) @ oracle.rope(k, 100, 1.0e4).T
+    b = oracle.rope(q, 50900, 1.0e4) @ oracle.rope(k, 50100, 1.0e4).T
+    assert abs(a - b).max() < 1e-9
+
+
+def test_round_io_matches_torch_casts():
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal(20000) * np.exp(rng.uniform(-8, 8, 20000))
+    # make some exact ties: value halfway between two bf16 numbers
+    t = torch.tensor([1.0, 1.0 + 2.0 ** -7, 3.0], dtype=torch.float64)
+    ties = (t + 2.0 ** -8 * torch.tensor([1.0, 1.0, 2.0], dtype=torch.float64)).numpy()
+    x = np.concatenate([x, ties, -ties])
+    got = oracle.round_io(x, True)
+    # a double that is exactly representable in fp32 casts to bf16 with one rounding in torch
+    xf = x.astype(np.float32).astype(np.float64)
+    same = xf == x
+    ref = torch.from_numpy(x.astype(np.float32)).to(torch.bfloat16).to(torch.float64).numpy()
+    assert same.sum() >= 6 and np.array_equal(got[same], ref[same])
+    # general doubles: result is a bf16 value and the nearest one
+    back = torch.from_numpy(got.astype(np.float32)).to(torch.bfloat16).to(torch.float64).numpy()
+    assert np.array_equal(back, got)
+    ulp = 2.0 ** (np.floor(np.log2(np.abs(x))) - 7)
+    assert np.all(np.abs(got - x) <= 0.5 * ulp * (1 + 1e-12))
+    assert np.array_equal(got, nearest_bf16(x))
+    assert np.array_equal(oracle.round_io(x, False), x.astype(np.float32).astype(np.float64))
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# O2 summaries (P11, P12, P14, P15 and a closed form)
+# ----------------------------------------------------------------------------------------------------------------
+def test_summary_all_high_is_mean_of_rotated_keys_P11():
+    w, q, k, v = small_problem(1, N=256, D=32)
+    for span in (64, 16):
+        s = oracle.summaries(k, span, 16, 7, w.rope_base)  # n_hi = D/2
+        kr = rope_complex(k, np.arange(7, 7 + 256), w.rope_base)
+        assert np.abs(s - kr.reshape(-1, span, 32).mean(1)).max() < 1e-12
+    # ... and then q.S_c is the mean of the chunk's q.k logits (closed form, linearity)
+    qr = rope_complex(q[0], np.arange(7, 7 + 256), w.rope_base)
+    s = oracle.summaries(k, 64, 16, 7, w.rope_base)
+    logits = qr[200] @ kr.T
+    assert np.abs(qr[200] @ s.T - logits.reshape(-1, 64).mean(1)).max() < 1e-11
+
+
+def test_summary_all_low_is_rotated_mean_of_raw_keys_P12():
+    w, q, k, v = small_problem(2, N=256, D=32)
+    for span in (64, 16):
+        s = oracle.summaries(k, span, 0, 11, w.rope_base)
+        raw_mean = k.astype(np.float64).reshape(-1, span, 32).mean(1)
+        p_mid = 11 + np.arange(256 // span) * span + (span - 1) / 2.0  # R2: centroid of the span's positions
+        assert np.abs(s - rope_complex(raw_mean, p_mid, w.rope_base)).max() < 1e-12
+
+
+def test_summary_mixed_rule_pairwise_split():
+    """Pairs < n_hi follow the 'rotate then average' rule, the others 'average then rotate'."""
+    w, q, k, v = small_problem(3, N=128, D=32)
+    n_hi = 5
+    s = oracle.summaries(k, 64, n_hi, 0, w.rope_base)
+    hi = oracle.summaries(k, 64, 16, 0, w.rope_base)
+    lo = oracle.summaries(k, 64, 0, 0, w.rope_base)
+    cols_hi = np.r_[0:n_hi, 16:16 + n_hi]
+    cols_lo = np.r_[n_hi:16, 16 + n_hi:32]
+    assert np.array_equal(s[:, cols_hi], hi[:, cols_hi]) and np.array_equal(s[:, cols_lo], lo[:, cols_lo])
+    # default rule R1: wavelength 2*pi/theta_i <= span
+    for D, base, span in ((64, 1e4, 64), (64, 1e4, 16), (128, 1e6, 64), (128, 1e6, 16)):
+        theta = base ** (-2.0 * np.arange(D // 2) / D)
+        assert oracle.default_n_hi(D, base, span) == int(np.sum(2 * np.pi / theta <= span))
+    assert np.array_equal(oracle.summaries(k, 64, -1, 0, w.rope_base),
+                          oracle.summaries(k, 64, oracle.default_n_hi(32, w.rope_base, 64), 0, w.rope_base))
+
+
+def test_summary_constant_key_closed_form():
+    """k_t = (1, 0) on every pair: rotate-then-average gives the Dirichlet kernel
+    e^{i p_mid th} * sin(S th/2) / (S sin(th/2)); average-then-rotate gives e^{i p_mid th}."""
+    D, S, base, pos0 = 16, 64, 100.0, 321
+    k = np.zeros((2 * S, D), dtype=np.float32)
+    k[:, : D // 2] = 1.0
+    theta = base ** (-2.0 * np.arange(D // 2) / D)
+    for n_hi in (D // 2, 0):
+        s = oracle.summaries(k, S, n_hi, pos0, base)
+        for sp in range(2):
+            p_mid = pos0 + sp * S + (S - 1) / 2.0
+            amp = np.sin(S * theta / 2) / (S * np.sin(theta / 2)) if n_hi else np.ones_like(theta)
+            z = amp * np.exp(1j * p_mid * theta)
+            assert np.abs(s[sp, : D // 2] - z.real).max() < 1e-12
+            assert np.abs(s[sp, D // 2:] - z.imag).max() < 1e-12
+
+
+def test_summary_chunk_group_consistency_P14_P15():
+    w, q, k, v = small_problem(4, N=256, D=32)
+    n_hi, pos0, h = 6, 40, 16
+    sc = oracle.summaries(k, 64, n_hi, pos0, w.rope_base)
+    sg = oracle.summaries(k, 16, n_hi, pos0, w.rope_base)
+    hi_cols = np.r_[0:n_hi, h:h + n_hi]
+    # pairs high at both levels: chunk summary = mean of its 4 group summaries
+    assert np.abs(sc[:, hi_cols] - sg.reshape(-1, 4, 32).mean(1)[:, hi_cols]).max() < 1e-12
+    # pairs low at both levels: un-rotating each summary at its own middle gives raw means, which nest
+    pm_c = pos0 + np.arange(4) * 64 + 31.5
+    pm_g = pos0 + np.arange(16) * 16 + 7.5
+    raw_c = rope_complex(sc, -pm_c, w.rope_base)
+    raw_g = rope_complex(sg, -pm_g, w.rope_base)
+    lo_cols = np.r_[n_hi:h, h + n_hi:32]
+    assert np.abs(raw_c[:, lo_cols] - raw_g.reshape(-1, 4, 32).mean(1)[:, lo_cols]).max() < 1e-12
+    # P15: the low-pair summary computed from ROTATED keys, (1/S) sum_t R(p_mid - p_t) k_rot_t
+    kr = rope_complex(k, pos0 + np.arange(256), w.rope_base)
+    for c in range(4):
+        acc = np.zeros(32)
+        for t in range(64):
+            acc += rope_complex(kr[c * 64 + t], pm_c[c] - (pos0 + c * 64 + t), w.rope_base)
+        assert np.abs(acc[lo_cols] / 64 - sc[c, lo_cols]).max() < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# O3 pooled query, O4/O5 routing (P8, P9, P10, P16, P17)
+# ----------------------------------------------------------------------------------------------------------------
+def test_pooled_query_linearity_P17():
+    w, q, k, v = small_problem(5, G=3, N=256, D=32)
+    qr = rope_complex(q, np.arange(256)[None].repeat(3, 0), w.rope_base)
+    qbar = oracle.pool_queries(qr, 64)
+    s = oracle.summaries(k, 64, -1, 0, w.rope_base)
+    per_query = np.einsum("gtd,cd->gtc", qr, s)  # every query's own score against every summary
+    mean_of_scores = per_query.reshape(3, 4, 64, 4).transpose(1, 0, 2, 3).reshape(4, 192, 4).mean(1)
+    assert np.abs(qbar @ s.T - mean_of_scores).max() < 1e-12
+    assert np.abs(qbar - qr.reshape(3, 4, 64, 32).mean(axis=(0, 2))).max() < 1e-13
+
+
+def brute_topk(scores, idxs, k):
+    order = np.lexsort((idxs, -scores))  # score descending, then index ascending
+    return np.sort(idxs[order[:k]])
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_topk_equals_bruteforce_sort_P8(seed):
+    rng = np.random.default_rng(seed)
+    n_b, D, F, L, Kc = 40, 8, 2, 3, 5
+    S_c = rng.integers(-3, 4, size=(n_b, D)).astype(np.float64)  # small integers -> many exact score ties
+    S_c[17] = S_c[9]
+    S_c[30] = S_c[9]
+    qbar = rng.integers(-2, 3, size=D).astype(np.float64)
+    for j in range(n_b):
+        idx, sc, cnt, alls = oracle.route_chunks(qbar, S_c, j, F, L, Kc)
+        cand = np.arange(F, max(F, j - max(L, 1)))
+        assert cnt == min(Kc, len(cand))
+        want = brute_topk(S_c[cand] @ qbar, cand, Kc) if len(cand) else np.array([], dtype=int)
+        assert np.array_equal(idx[:cnt], want) and np.all(idx[cnt:] == -1)
+        assert np.array_equal(sc[:cnt], S_c[idx[:cnt]] @ qbar)
+        assert np.array_equal(np.isfinite(alls), np.isin(np.arange(n_b), cand))
+        # group level: brute force over the C/gs groups of the selected chunks
+        gpc, Kg = 4, 7
+        S_g = rng.integers(-3, 4, size=(n_b * gpc, D)).astype(np.float64)
+        gidx, gsc, gcnt, cs = oracle.route_groups(qbar, S_g, gpc, idx[:cnt], Kg)
+        gcand = (idx[:cnt, None] * gpc + np.arange(gpc)[None]).reshape(-1)
+        assert gcnt == min(Kg, len(gcand))
+        gwant = brute_topk(S_g[gcand] @ qbar, gcand, Kg) if len(gcand) else np.array([], dtype=int)
+        assert np.array_equal(gidx[:gcnt], gwant) and np.all(gidx[gcnt:] == -1)
+
+
+def test_routing_invariances_P9_P10_P16():
+    w, q, k, v = small_problem(6, G=2, N=1024, D=32, clustered=True)
+    p = oracle.OracleParams(G=2, N=1024, D=32, F=1, L=1, Kc=3, Kg=5, base=w.rope_base)
+    r0 = oracle.prefill_slice(p, q, k, v, attend=False)
+    # P9: scaling Q by a power of two changes no index set
+    r1 = oracle.prefill_slice(p, q * np.float32(4.0), k, v, attend=False)
+    assert np.array_equal(r0.chunk_idx, r1.chunk_idx) and np.array_equal(r0.group_idx, r1.group_idx)
+    # P16: a global position shift leaves scores and index sets unchanged (RoPE is relative)
+    p2 = oracle.OracleParams(**{**p.__dict__, "pos0": 4096})
+    r2 = oracle.prefill_slice(p2, q, k, v, attend=False)
+    assert np.array_equal(r0.chunk_idx, r2.chunk_idx) and np.array_equal(r0.group_idx, r2.group_idx)
+    assert np.nanmax(np.abs(r0.chunk_all_scores - r2.chunk_all_scores)) < 1e-9
+    # P10: K_g = (C/gs)*K_c opens every group of every selected chunk (the "exact-token variant")
+    p3 = oracle.OracleParams(**{**p.__dict__, "Kg": 12})
+    r3 = oracle.prefill_slice(p3, q, k, v, attend=False)
+    for b in range(16):
+        ch = r3.chunk_idx[b][r3.chunk_idx[b] >= 0]
+        want = (ch[:, None] * 4 + np.arange(4)[None]).reshape(-1)
+        assert np.array_equal(r3.group_idx[b][: r3.n_groups[b]], want)
+    # selected chunks are middle chunks only; sets are ascending and distinct
+    for b in range(16):
+        ch = r0.chunk_idx[b][: r0.n_chunks[b]]
+        assert np.all(ch >= p.F) and np.all(ch < b - 1) and np.all(np.diff(ch) > 0)
+        assert r0.n_chunks[b] == min(p.Kc, max(0, b - 1 - p.F))
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# union set (P6, P7) and the numbers the paper prints
+# ----------------------------------------------------------------------------------------------------------------
+def test_union_set_contains_sink_local_current_and_paper_sizes_P6_P7():
+    g = golden()
+    C, gs = int(g["chunk_size"]), int(g["group_size"])
+    F, L = int(g["needle_keep_first"]), int(g["needle_keep_last"])
+    Kc, Kg = int(g["needle_topk_chunks"]), int(g["needle_topk_groups"])
+    n_tok = int(g["needle_prompt_tokens"])
+    n_chunks = -(-n_tok // C)
+    assert n_chunks == int(g["needle_chunks"])
+    j = n_chunks - 1
+    rng = np.random.default_rng(0)
+    # any K_g distinct middle groups (middle = chunks F .. j-L-1)
+    groups = rng.choice(np.arange(F * 4, (j - L) * 4), size=Kg, replace=False)
+    vis = oracle.key_set(j, C, gs, F, L, groups)
+    assert vis[: F * C].all() and vis[(j - L) * C: j * C].all() and vis[j * C:].all()  # P6
+    for gi in groups:
+        assert vis[gi * gs:(gi + 1) * gs].all()
+    assert vis.sum() == Kg * gs + (F + L + 1) * C == 1216  # P7
+    assert round(100.0 * vis.sum() / n_tok, 1) == g["needle_sparsity_percent"]  # "approximately 1.9%"
+    # the Qwen3 exact-token budget: K_c = 16 whole chunks -> 1024 routed tokens
+    chunks16 = rng.choice(np.arange(2, j - 8), size=16, replace=False)
+    groups16 = (chunks16[:, None] * 4 + np.arange(4)[None]).reshape(-1)
+    vis16 = oracle.key_set(j, C, gs, 2, 8, groups16)
+    assert vis16.sum() - (2 + 8 + 1) * C == int(g["qwen3_routed_budget_tokens"])
+    # early blocks: sink and local overlap -> union, never double counted (R13)
+    assert oracle.key_set(1, C, gs, 2, 8, []).sum() == 2 * C
+    assert oracle.key_set(0, C, gs, 2, 8, []).sum() == C
+    # -1 padding is ignored; future / current / duplicate / negative groups are rejected
+    assert oracle.key_set(5, C, gs, 1, 1, [-1, 8, -1]).sum() == 3 * C + gs
+    for bad in ([20], [24], [8, 8], [-2]):
+        with pytest.raises(ValueError):
+            oracle.key_set(5, C, gs, 1, 1, bad)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# O6 attention (P1..P5)
+# ----------------------------------------------------------------------------------------------------------------
+def test_full_coverage_equals_dense_causal_sdpa_P1():
+    """PAPER.md:281 / Table 7: full chunk coverage must reproduce dense causal SDPA (< 1e-6)."""
+    tol = golden()["full_coverage_max_abs"]
+    for seed, (G, N, D, base) in enumerate([(2, 512, 32, 1.0e4), (4, 1024, 64, 1.0e4)]):
+        w, q, k, v = small_problem(seed, G=G, N=N, D=D, base=base)
+        p = oracle.OracleParams(G=G, N=N, D=D, F=1, L=1, Kc=N // 64, Kg=N // 16, base=base)
+        r = oracle.prefill_slice(p, q, k, v)
+        pos = np.arange(N)
+        ref = sdpa_causal(rope_complex(q, pos[None].repeat(G, 0), base), rope_complex(k, pos, base), v)
+        got = r.out.transpose(1, 0, 2, 3).reshape(G, N, D)
+        assert np.abs(got - ref).max() < tol
+        # the oracle's own Eq. (1) helper agrees with torch SDPA too
+        kr = oracle.round_io(oracle.rope(k, 0, base), False)
+        qb = oracle.round_io(oracle.rope(q[:, 128:192], 128, base), False)
+        d_out, _ = oracle.dense_block(qb, kr, v.astype(np.float64), 2, 64)
+        assert np.abs(d_out - ref[:, 128:192]).max() < tol
+
+
+def test_early_blocks_equal_dense_for_any_budget_P2():
+    w, q, k, v = small_problem(7, G=2, N=512, D=32)
+    pos = np.arange(512)
+    ref = sdpa_causal(rope_complex(q, pos[None].repeat(2, 0), w.rope_base), rope_complex(k, pos, w.rope_base), v)
+    for F, L in ((1, 1), (2, 3), (0, 0)):
+        p = oracle.OracleParams(G=2, N=512, D=32, F=F, L=L, Kc=0, Kg=0, base=w.rope_base)
+        r = oracle.prefill_slice(p, q, k, v)
+        n_dense = F + max(L, 1) + 1  # blocks 0 .. F+L_eff see every earlier token
+        got = r.out.transpose(1, 0, 2, 3).reshape(2, 512, 32)
+        assert np.abs(got[:, : n_dense * 64] - ref[:, : n_dense * 64]).max() < 1e-6
+        assert np.abs(got[:, n_dense * 64:] - ref[:, n_dense * 64:]).max() > 1e-4  # later blocks really are sparse
+
+
+def test_softmax_rows_sum_to_one_and_lse_P3():
+    w, q, k, v = small_problem(8, G=2, N=512, D=32)
+    p = oracle.OracleParams(G=2, N=512, D=32, Kc=2, Kg=3, base=w.rope_base)
+    ones = np.ones_like(v)
+    r = oracle.prefill_slice(p, q, k, ones)
+    assert np.abs(r.out - 1.0).max() < 1e-14  # sum_j softmax_j * 1 == 1
+    assert np.isfinite(r.lse).all()
+    # lse against torch.logsumexp over the block's visible set
+    j = 6
+    vis = oracle.key_set(j, 64, 16, 1, 1, r.group_idx[j])
+    kr = rope_complex(k, np.arange(512), w.rope_base).astype(np.float32).astype(np.float64)
+    qr = rope_complex(q[1, j * 64: j * 64 + 64], np.arange(j * 64, j * 64 + 64), w.rope_base)
+    qr = qr.astype(np.float32).astype(np.float64)
+    for row in (0, 17, 63):
+        keys = np.nonzero(vis[: j * 64 + row + 1])[0]
+        logits = torch.from_numpy(qr[row] @ kr[keys].T / math.sqrt(32))
+        assert abs(float(torch.logsumexp(logits, 0)) - r.lse[j, 1, row]) < 1e-12
+
+
+def test_attention_against_direct_softmax_on_visible_set():
+    """O6 on a sparse set, checked row by row with torch.softmax over the explicitly enumerated key set."""
+    w, q, k, v = small_problem(9, G=2, N=512, D=32, clustered=True)
+    p = oracle.OracleParams(G=2, N=512, D=32, Kc=2, Kg=3, base=w.rope_base, io_bf16=True)
+    r = oracle.prefill_slice(p, q, k, v)
+    to_bf16 = nearest_bf16
+    kr = to_bf16(rope_complex(k, np.arange(512), w.rope_base))
+    for j in (0, 1, 3, 7):
+        vis = oracle.key_set(j, 64, 16, 1, 1, r.group_idx[j])
+        for h in range(2):
+            qr = to_bf16(rope_complex(q[h, j * 64: j * 64 + 64], np.arange(j * 64, j * 64 + 64), w.rope_base))
+            for row in (0, 31, 63):
+                keys = np.nonzero(vis[: j * 64 + row + 1])[0]
+                pw = torch.softmax(torch.from_numpy(qr[row] @ kr[keys].T / math.sqrt(32)), 0).numpy()
+                assert np.abs(pw @ v[keys].astype(np.float64) - r.out[j, h, row]).max() < 1e-12
+
+
+def test_index_list_permutation_invariance_P4():
+    w, q, k, v = small_problem(10, G=1, N=512, D=32)
+    kr = oracle.rope(k, 0, w.rope_base)
+    qb = oracle.rope(q[:, 448:512], 448, w.rope_base)
+    groups = np.array([5, 9, 10, 17, 22, -1, -1], dtype=np.int32)
+    a, la, na = oracle.attend_block(qb, kr, v, 7, 64, 16, 1, 1, groups)
+    b, lb, nb = oracle.attend_block(qb, kr, v, 7, 64, 16, 1, 1, groups[::-1].copy())
+    assert np.abs(a - b).max() < 1e-15 and np.array_equal(na, nb)
+    assert np.array_equal(na, 5 * 16 + 2 * 64 + np.arange(1, 65))  # row r sees r+1 current tokens (causal)
+
+
+def test_causality_P5():
+    """Perturbing tokens after position t changes neither output row t nor any index set of earlier blocks."""
+    w, q, k, v = small_problem(11, G=2, N=512, D=32)
+    p = oracle.OracleParams(G=2, N=512, D=32, Kc=2, Kg=3, base=w.rope_base)
+    r0 = oracle.prefill_slice(p, q, k, v)
+    t = 300  # inside block 4
+    q2, k2, v2 = q.copy(), k.copy(), v.copy()
+    q2[:, t + 1:] += 1.0
+    k2[t + 1:] -= 2.0
+    v2[t + 1:] *= 3.0
+    r1 = oracle.prefill_slice(p, q2, k2, v2)
+    jb, row = divmod(t, 64)
+    assert np.array_equal(r0.out[:jb], r1.out[:jb])
+    assert np.array_equal(r0.out[jb, :, : row + 1], r1.out[jb, :, : row + 1])
+    assert not np.array_equal(r0.out[jb, :, row + 1:], r1.out[jb, :, row + 1:])
+    assert np.array_equal(r0.chunk_idx[:jb], r1.chunk_idx[:jb]) and np.array_equal(r0.group_idx[:jb], r1.group_idx[:jb])
+
+
+def test_bad_inputs_are_rejected():
+    w, q, k, v = small_problem(12, G=1, N=128, D=32)
+    p = oracle.OracleParams(G=1, N=128, D=32, base=w.rope_base)
+    k2 = k.copy()
+    k2[3, 3] = np.nan
+    with pytest.raises(ValueError):
+        oracle.prefill_slice(p, q, k2, v)
+    with pytest.raises(ValueError):  # R12: partial last chunk is not a closed chunk
+        oracle.prefill_slice(oracle.OracleParams(G=1, N=100, D=32), q[:, :100], k[:100], v[:100])
+
+
+def test_config1_tiny_cpu_checkable():
+    """BASELINE.json configs[0]: runs in seconds; top-k = all chunks equals dense causal attention."""
+    w = W.get("c1")
+    q, k, v = W.generate(w, 0)
+    p = oracle.params_from_workload(w)
+    r = oracle.prefill_slice(p, q[0], k[0, 0], v[0, 0])
+    assert r.out.shape == (16, 4, 64, 64)
+    assert np.all(r.n_chunks == np.minimum(4, np.maximum(0, np.arange(16) - 2)))
+    assert np.all(r.n_groups == np.minimum(8, 4 * r.n_chunks))
+    p_all = oracle.OracleParams(**{**p.__dict__, "Kc": 16, "Kg": 64})
+    r_all = oracle.prefill_slice(p_all, q[0], k[0, 0], v[0, 0])
+    pos = np.arange(1024)
+    ref = sdpa_causal(rope_complex(q[0], pos[None].repeat(4, 0), 1e4), rope_complex(k[0, 0], pos, 1e4), v[0, 0])
+    assert np.abs(r_all.out.transpose(1, 0, 2, 3).reshape(4, 1024, 64) - ref).max() < 1e-6
