@@ -1,0 +1,270 @@
+// C-ABI entry points: host-side validation and dispatch only.  All arithmetic of the path runs in the kernels.
+#include <math.h>
+#include <new>
+#include <string.h>
+
+#include "hga_common.cuh"
+
+namespace hga {
+
+static int default_n_hi(int D, double base, int span) {
+  // Reading R1: pair i is "high-frequency" iff its wavelength 2*pi/theta_i is <= the span length.
+  int n = 0;
+  for (int i = 0; i < D / 2; ++i) {
+    double theta = pow(base, -2.0 * (double)i / (double)D);
+    if (kTwoPi / theta <= (double)span) ++n;
+  }
+  return n;
+}
+
+hga_status validate(const hga_params* p) {
+  if (!p) return HGA_ERR_INVALID_ARG;
+  if (p->batch <= 0 || p->seq <= 0 || p->n_q_heads <= 0 || p->n_kv_heads <= 0 || p->head_dim <= 0)
+    return HGA_ERR_INVALID_ARG;
+  if (p->n_q_heads % p->n_kv_heads) return HGA_ERR_INVALID_ARG;
+  if (p->chunk <= 0 || p->group <= 0 || p->chunk % p->group) return HGA_ERR_INVALID_ARG;
+  if (p->seq % p->chunk) return HGA_ERR_INVALID_ARG;  // only closed chunks are summarised
+  if (p->n_sink < 0 || p->n_local < 0 || p->topk_chunks < 0 || p->topk_groups < 0) return HGA_ERR_INVALID_ARG;
+  if (p->n_hi_chunk < -1 || p->n_hi_group < -1 || p->n_hi_chunk > p->head_dim / 2 || p->n_hi_group > p->head_dim / 2)
+    return HGA_ERR_INVALID_ARG;
+  if (!(p->rope_base > 0.0) || !isfinite(p->rope_base)) return HGA_ERR_INVALID_ARG;
+  if (!(p->softmax_scale >= 0.0f) || !isfinite(p->softmax_scale)) return HGA_ERR_INVALID_ARG;
+  if (p->io_dtype != HGA_F32 && p->io_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
+  if (p->out_dtype != HGA_F32 && p->out_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
+  if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05) return HGA_ERR_INVALID_ARG;
+  if (p->reserved != 0) return HGA_ERR_INVALID_ARG;
+  if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
+  // what the kernels implement
+  if (p->chunk != kChunk) return HGA_ERR_UNSUPPORTED;
+  if (p->group % 16) return HGA_ERR_UNSUPPORTED;
+  if (p->head_dim != 64 && p->head_dim != 128) return HGA_ERR_UNSUPPORTED;
+  if (p->attend_impl == HGA_ATTEND_TCGEN05 && p->io_dtype != HGA_BF16) return HGA_ERR_UNSUPPORTED;
+  if ((long long)p->topk_groups * (p->group / 16) + (long long)(p->n_sink + p->n_local + 2) * 4 > 40000)
+    return HGA_ERR_UNSUPPORTED;  // key list must fit in shared memory
+  if ((long long)p->seq / p->chunk > 32768) return HGA_ERR_UNSUPPORTED;
+  return HGA_OK;
+}
+
+hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
+  hga_status st = validate(p);
+  if (st != HGA_OK) return st;
+  d->B = p->batch; d->N = p->seq; d->Hq = p->n_q_heads; d->Hkv = p->n_kv_heads; d->G = p->n_q_heads / p->n_kv_heads;
+  d->D = p->head_dim; d->half = p->head_dim / 2;
+  d->C = p->chunk; d->gs = p->group; d->gpc = p->chunk / p->group;
+  d->n_b = p->seq / p->chunk; d->n_g = p->seq / p->group;
+  d->F = p->n_sink; d->L = p->n_local; d->L_eff = p->n_local > 1 ? p->n_local : 1;
+  d->Kc = p->topk_chunks; d->Kg = p->topk_groups;
+  d->n_hi_c = p->n_hi_chunk >= 0 ? p->n_hi_chunk : default_n_hi(p->head_dim, p->rope_base, p->chunk);
+  d->n_hi_g = p->n_hi_group >= 0 ? p->n_hi_group : default_n_hi(p->head_dim, p->rope_base, p->group);
+  d->pos0 = p->pos0;
+  d->scale = p->softmax_scale > 0.0f ? p->softmax_scale : (float)(1.0 / sqrt((double)p->head_dim));
+  d->bf16_io = p->io_dtype == HGA_BF16;
+  d->bf16_out = p->out_dtype == HGA_BF16;
+  if (f) {
+    for (int i = 0; i < kMaxHalfDim; ++i) f->turns[i] = 0.0;
+    for (int i = 0; i < d->half; ++i) f->turns[i] = pow(p->rope_base, -2.0 * (double)i / (double)p->head_dim) / kTwoPi;
+  }
+  return HGA_OK;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static size_t score_ws_bytes(const Derived& d) {
+  return (size_t)d.B * d.Hkv * d.n_b * d.n_b * sizeof(float);
+}
+
+}  // namespace hga
+
+using namespace hga;
+
+extern "C" {
+
+const char* hga_status_string(hga_status s) {
+  switch (s) {
+    case HGA_OK: return "HGA_OK";
+    case HGA_ERR_INVALID_ARG: return "HGA_ERR_INVALID_ARG: null pointer, bad shape or misaligned pointer";
+    case HGA_ERR_UNSUPPORTED: return "HGA_ERR_UNSUPPORTED: valid request the sm_100a kernels do not implement";
+    case HGA_ERR_WORKSPACE: return "HGA_ERR_WORKSPACE: workspace missing or too small";
+    case HGA_ERR_CUDA: return "HGA_ERR_CUDA: CUDA runtime or launch failure (or no device)";
+  }
+  return "HGA: unknown status";
+}
+
+int32_t hga_version(void) { return 100; }
+
+int32_t hga_default_n_hi(int32_t head_dim, double rope_base, int32_t span) {
+  if (head_dim <= 0 || (head_dim & 1) || !(rope_base > 0.0) || span <= 0) return -1;
+  return default_n_hi(head_dim, rope_base, span);
+}
+
+hga_status hga_validate(const hga_params* p) { return validate(p); }
+
+hga_status hga_workspace_bytes(const hga_params* p, size_t* bytes) {
+  if (!bytes) return HGA_ERR_INVALID_ARG;
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  *bytes = score_ws_bytes(d);
+  return HGA_OK;
+}
+
+hga_status hga_rope(const hga_params* p, const void* x_raw, int32_t n_heads, void* x_rot, float* pooled,
+                    void* stream) {
+  Derived d;
+  RopeFreq f;
+  hga_status st = derive(p, &d, &f);
+  if (st != HGA_OK) return st;
+  if (!x_raw || !x_rot || n_heads <= 0 || !aligned16(x_raw) || !aligned16(x_rot) || !aligned16(pooled))
+    return HGA_ERR_INVALID_ARG;
+  if (pooled && (n_heads % d.Hkv)) return HGA_ERR_INVALID_ARG;
+  return launch_rope(d, f, x_raw, n_heads, x_rot, pooled, (cudaStream_t)stream);
+}
+
+hga_status hga_build_summaries(const hga_params* p, const void* k_raw, void* k_rot, float* chunk_sum,
+                               float* group_sum, void* stream) {
+  Derived d;
+  RopeFreq f;
+  hga_status st = derive(p, &d, &f);
+  if (st != HGA_OK) return st;
+  if (!k_raw || !aligned16(k_raw) || !aligned16(k_rot) || !aligned16(chunk_sum) || !aligned16(group_sum))
+    return HGA_ERR_INVALID_ARG;
+  return launch_summaries(d, f, k_raw, k_rot, chunk_sum, group_sum, (cudaStream_t)stream);
+}
+
+hga_status hga_route(const hga_params* p, const float* q_pooled, const float* chunk_sum, const float* group_sum,
+                     int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx, float* group_score,
+                     int32_t* n_groups, void* workspace, size_t workspace_bytes, void* stream) {
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  if (!q_pooled || !chunk_sum || !chunk_idx) return HGA_ERR_INVALID_ARG;
+  if (d.Kg > 0 && (!group_sum || !group_idx)) return HGA_ERR_INVALID_ARG;
+  if (!aligned16(q_pooled) || !aligned16(chunk_sum) || !aligned16(group_sum)) return HGA_ERR_INVALID_ARG;
+  if (!workspace || !aligned16(workspace) || workspace_bytes < score_ws_bytes(d)) return HGA_ERR_WORKSPACE;
+  return launch_route(d, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
+                      n_groups, (float*)workspace, (cudaStream_t)stream);
+}
+
+hga_status hga_attend(const hga_params* p, const void* q_rot, const void* k_rot, const void* v,
+                      const int32_t* group_idx, void* out, float* lse, void* stream) {
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  if (!q_rot || !k_rot || !v || !out) return HGA_ERR_INVALID_ARG;
+  if (d.Kg > 0 && !group_idx) return HGA_ERR_INVALID_ARG;
+  if (!aligned16(q_rot) || !aligned16(k_rot) || !aligned16(v) || !aligned16(out)) return HGA_ERR_INVALID_ARG;
+  int impl = p->attend_impl;
+  if (impl == HGA_ATTEND_AUTO) impl = d.bf16_io ? HGA_ATTEND_TCGEN05 : HGA_ATTEND_SIMT;
+  if (impl == HGA_ATTEND_TCGEN05)
+    return launch_attend_tc(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
+  return launch_attend_simt(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
+}
+
+hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) {
+  if (!b) return HGA_ERR_INVALID_ARG;
+  hga_status st = hga_rope(p, b->q_raw, p ? p->n_q_heads : 0, b->q_rot, b->q_pooled, stream);
+  if (st != HGA_OK) return st;
+  if (!b->q_pooled || !b->k_rot || !b->chunk_sum) return HGA_ERR_INVALID_ARG;
+  st = hga_build_summaries(p, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum, stream);
+  if (st != HGA_OK) return st;
+  st = hga_route(p, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
+                 b->group_score, b->n_groups, b->workspace, b->workspace_bytes, stream);
+  if (st != HGA_OK) return st;
+  return hga_attend(p, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, stream);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Host-buffer path
+// ---------------------------------------------------------------------------------------------------------------
+struct hga_host_plan {
+  hga_params p;
+  Derived d;
+  cudaStream_t stream;
+  void* arena;
+  size_t arena_bytes;
+  hga_buffers buf;
+  size_t q_bytes, kv_bytes, out_bytes, gidx_bytes, lse_bytes;
+};
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+hga_status hga_host_bytes(const hga_params* p, int32_t with_group_idx, int32_t with_lse, size_t* h2d, size_t* d2h) {
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  size_t e = d.bf16_io ? 2 : 4, eo = d.bf16_out ? 2 : 4;
+  size_t q = (size_t)d.B * d.Hq * d.N * d.D, kv = (size_t)d.B * d.Hkv * d.N * d.D;
+  if (h2d) *h2d = (q + 2 * kv) * e;
+  if (d2h)
+    *d2h = q * eo + (with_group_idx ? (size_t)d.B * d.Hkv * d.n_b * d.Kg * 4 : 0) +
+           (with_lse ? (size_t)d.B * d.Hq * d.N * 4 : 0);
+  return HGA_OK;
+}
+
+hga_status hga_host_plan_create(const hga_params* p, hga_host_plan** out_plan) {
+  if (!out_plan) return HGA_ERR_INVALID_ARG;
+  *out_plan = nullptr;
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  hga_host_plan* pl = new (std::nothrow) hga_host_plan();
+  if (!pl) return HGA_ERR_CUDA;
+  pl->p = *p;
+  pl->d = d;
+  size_t e = d.bf16_io ? 2 : 4, eo = d.bf16_out ? 2 : 4;
+  size_t q = (size_t)d.B * d.Hq * d.N * d.D, kv = (size_t)d.B * d.Hkv * d.N * d.D;
+  size_t units = (size_t)d.B * d.Hkv * d.n_b;
+  pl->q_bytes = q * e; pl->kv_bytes = kv * e; pl->out_bytes = q * eo;
+  pl->gidx_bytes = units * (d.Kg > 0 ? d.Kg : 1) * 4; pl->lse_bytes = (size_t)d.B * d.Hq * d.N * 4;
+  size_t sizes[] = {pl->q_bytes, pl->kv_bytes, pl->kv_bytes, units * d.D * 4, units * d.D * 4,
+                    (size_t)d.B * d.Hkv * d.n_g * d.D * 4, units * (d.Kc > 0 ? d.Kc : 1) * 4, pl->gidx_bytes,
+                    pl->out_bytes, pl->lse_bytes, score_ws_bytes(d)};
+  size_t total = 0;
+  for (size_t s : sizes) total += align_up(s);
+  pl->arena_bytes = total;
+  if (cudaMalloc(&pl->arena, total) != cudaSuccess) { delete pl; return HGA_ERR_CUDA; }
+  if (cudaStreamCreateWithFlags(&pl->stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaFree(pl->arena); delete pl; return HGA_ERR_CUDA;
+  }
+  char* base = (char*)pl->arena;
+  size_t off = 0;
+  auto take = [&](size_t s) { void* r = base + off; off += align_up(s); return r; };
+  hga_buffers& b = pl->buf;
+  memset(&b, 0, sizeof(b));
+  void* dq = take(sizes[0]); void* dk = take(sizes[1]); void* dv = take(sizes[2]);
+  b.q_raw = dq; b.q_rot = dq; b.k_raw = dk; b.k_rot = dk; b.v = dv;   // RoPE in place
+  b.q_pooled = (float*)take(sizes[3]); b.chunk_sum = (float*)take(sizes[4]); b.group_sum = (float*)take(sizes[5]);
+  b.chunk_idx = (int32_t*)take(sizes[6]); b.group_idx = (int32_t*)take(sizes[7]);
+  b.out = take(sizes[8]); b.lse = (float*)take(sizes[9]);
+  b.workspace = take(sizes[10]); b.workspace_bytes = sizes[10];
+  *out_plan = pl;
+  return HGA_OK;
+}
+
+hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k_host, const void* v_host,
+                            void* out_host, int32_t* group_idx_host, float* lse_host) {
+  if (!pl || !q_host || !k_host || !v_host || !out_host) return HGA_ERR_INVALID_ARG;
+  cudaStream_t s = pl->stream;
+  HGA_CUDA_OK(cudaMemcpyAsync((void*)pl->buf.q_raw, q_host, pl->q_bytes, cudaMemcpyHostToDevice, s));
+  HGA_CUDA_OK(cudaMemcpyAsync((void*)pl->buf.k_raw, k_host, pl->kv_bytes, cudaMemcpyHostToDevice, s));
+  HGA_CUDA_OK(cudaMemcpyAsync((void*)pl->buf.v, v_host, pl->kv_bytes, cudaMemcpyHostToDevice, s));
+  hga_buffers b = pl->buf;
+  if (!lse_host) b.lse = nullptr;
+  hga_status st = hga_prefill(&pl->p, &b, (void*)s);
+  if (st != HGA_OK) return st;
+  HGA_CUDA_OK(cudaMemcpyAsync(out_host, pl->buf.out, pl->out_bytes, cudaMemcpyDeviceToHost, s));
+  if (group_idx_host && pl->d.Kg > 0)
+    HGA_CUDA_OK(cudaMemcpyAsync(group_idx_host, pl->buf.group_idx, pl->gidx_bytes, cudaMemcpyDeviceToHost, s));
+  if (lse_host) HGA_CUDA_OK(cudaMemcpyAsync(lse_host, pl->buf.lse, pl->lse_bytes, cudaMemcpyDeviceToHost, s));
+  HGA_CUDA_OK(cudaStreamSynchronize(s));
+  return HGA_OK;
+}
+
+void hga_host_plan_destroy(hga_host_plan* pl) {
+  if (!pl) return;
+  cudaStreamDestroy(pl->stream);
+  cudaFree(pl->arena);
+  delete pl;
+}
+
+}  // extern "C"

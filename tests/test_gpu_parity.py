@@ -1,0 +1,192 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI binding, against the CPU oracle on the same
+seeded inputs.  Element-by-element at sizes the oracle finishes in seconds; sampled blocks at BASELINE.json's full
+sizes in the launch configuration bench.py times.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import hga_workloads as W
+import oracle
+import paper_2606_30709_b200 as hga
+from paper_2606_30709_b200.binding import ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, HGA_BF16, HGA_F32
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _all_slices(w):
+    return [(b, kh) for b in range(w.batch) for kh in range(w.n_kv_heads)]
+
+
+def _sample_blocks(n_b, n, seed):
+    """first blocks (dense regime, partial budgets), a ragged middle sample, and the last block."""
+    rng = np.random.default_rng(seed)
+    fixed = [0, 1, 2, 3, 4, 5, n_b // 2, n_b - 2, n_b - 1]
+    extra = rng.choice(np.arange(6, n_b - 2), size=max(0, n - len(fixed)), replace=False).tolist() if n_b > 16 else []
+    return sorted(set(j for j in fixed + extra if 0 <= j < n_b))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 1: tiny, fp32, every element, three seeds; SIMT fp32 kernel (the 1e-4 path)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_c1_full_parity_fp32(seed):
+    w = W.get("c1")
+    q, k, v = W.generate(w, seed)
+    p, buf = parity.run_gpu(w, q, k, v)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks)
+    assert rep["worst"]["out"] <= 1e-4
+
+
+def test_c1_topk_all_equals_dense_causal():
+    """BASELINE.json configs[0]: 'also run with top-k = all chunks, which must equal dense causal attention'."""
+    w = W.get("c1")
+    q, k, v = W.generate(w, 0)
+    p, buf = parity.run_gpu(w, q, k, v, topk_chunks=16, topk_groups=64)
+    op = dataclasses.replace(oracle.params_from_workload(w), Kc=16, Kg=64)
+    kr = oracle.round_io(oracle.rope(k[0, 0], 0, w.rope_base), False)
+    got = buf.out[0].cpu().numpy().astype(np.float64)
+    for j in range(w.n_blocks):
+        qb = oracle.round_io(oracle.rope(q[0, :, j * 64:(j + 1) * 64], j * 64, w.rope_base), False)
+        ref, _ = oracle.dense_block(qb, kr, v[0, 0].astype(np.float64), j, 64)
+        assert np.abs(got[:, j * 64:(j + 1) * 64] - ref).max() <= 1e-4
+    # and against torch SDPA on the GPU's own rotated tensors (secondary sanity check, not the oracle)
+    v_dev = torch.from_numpy(v).cuda().expand(-1, 4, -1, -1)
+    ref2 = torch.nn.functional.scaled_dot_product_attention(buf.q_rot, buf.k_rot.expand(-1, 4, -1, -1), v_dev,
+                                                            is_causal=True)
+    assert (buf.out - ref2).abs().max().item() <= 1e-4
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# small bf16 problems covering ragged tails, G in {1, 2, 3, 8}, D in {64, 128}, both attend kernels
+# ---------------------------------------------------------------------------------------------------------------
+SMALL = [
+    # name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L
+    ("d64_g1", 2, 1024, 4, 4, 64, 1e4, 4, 9, 1, 1),
+    ("d128_g8", 1, 2048, 16, 2, 128, 1e6, 6, 24, 1, 1),
+    ("d128_g3", 1, 1536, 6, 2, 128, 1e6, 5, 7, 2, 3),
+    ("d64_g2_nolocal", 1, 1024, 4, 2, 64, 1e4, 3, 5, 0, 0),
+    ("d128_g2_pos0", 1, 1024, 4, 2, 128, 1e6, 4, 16, 1, 2),
+]
+
+
+@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05])
+@pytest.mark.parametrize("cfg", SMALL, ids=[c[0] for c in SMALL])
+def test_small_bf16_full_parity(cfg, impl):
+    name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L = cfg
+    w = W.Workload(name, B, N, Hq, Hkv, D, "bf16", base, n_sink=F, n_local=L, topk_chunks=Kc, topk_groups=Kg,
+                   n_clusters=8, pos0=(40000 if "pos0" in name else 0))
+    q, k, v = W.generate(w, 7)
+    p, buf = parity.run_gpu(w, q, k, v, attend_impl=impl)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks * B * Hkv)
+
+
+@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05])
+def test_bf16_full_coverage_equals_dense(impl):
+    """full chunk coverage must reproduce dense causal attention (bf16 bar: 2e-2)."""
+    w = W.Workload("dense", 1, 1024, 8, 2, 128, "bf16", 1e6, topk_chunks=16, topk_groups=64, n_clusters=4)
+    q, k, v = W.generate(w, 3)
+    p, buf = parity.run_gpu(w, q, k, v, attend_impl=impl)
+    kr = oracle.round_io(oracle.rope(k[0], 0, w.rope_base), True)
+    got = buf.out[0].cpu().numpy().astype(np.float64)
+    for kh in range(2):
+        for j in (0, 1, 7, 15):
+            qb = oracle.round_io(oracle.rope(q[0, kh * 4:(kh + 1) * 4, j * 64:(j + 1) * 64], j * 64, w.rope_base), True)
+            ref, _ = oracle.dense_block(qb, kr[kh], v[0, kh].astype(np.float64), j, 64)
+            assert np.abs(got[kh * 4:(kh + 1) * 4, j * 64:(j + 1) * 64] - ref).max() <= 2e-2
+
+
+@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05])
+def test_attend_isolated_caller_supplied_lists(impl):
+    """S4 alone: oracle-rotated Q/K and arbitrary (unsorted, padded, window-overlapping) group lists."""
+    w = W.Workload("iso", 1, 1024, 4, 2, 128, "bf16", 1e6, topk_chunks=4, topk_groups=12, n_clusters=4)
+    q, k, v = W.generate(w, 11)
+    rng = np.random.default_rng(5)
+    G, C = 2, 64
+    q_rot = np.stack([oracle.round_io(oracle.rope(q[0, h], 0, w.rope_base), True) for h in range(4)])[None]
+    k_rot = np.stack([oracle.round_io(oracle.rope(k[0, h], 0, w.rope_base), True) for h in range(2)])[None]
+    gidx = -np.ones((1, 2, 16, 12), dtype=np.int32)
+    for kh in range(2):
+        for j in range(16):
+            n_avail = 4 * j
+            take = min(n_avail, int(rng.integers(0, 11)))
+            if take:
+                sel = rng.choice(n_avail, size=take, replace=False)  # may fall inside sink/local windows: set union
+                slots = rng.choice(12, size=take, replace=False)     # -1 holes anywhere, unsorted
+                gidx[0, kh, j, slots] = sel
+    p = hga.params_from_workload(w, attend_impl=impl)
+    dev = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dt)
+    out, lse = hga.hga_attend(p, dev(q_rot.astype(np.float32), torch.bfloat16), dev(k_rot.astype(np.float32), torch.bfloat16),
+                              dev(v, torch.bfloat16), dev(gidx, torch.int32))
+    torch.cuda.synchronize()
+    out, lse = out.cpu().numpy(), lse.cpu().numpy()
+    for kh in range(2):
+        for j in range(16):
+            ref, rl, _ = oracle.attend_block(q_rot[0, kh * G:(kh + 1) * G, j * C:(j + 1) * C], k_rot[0, kh],
+                                             v[0, kh].astype(np.float64), j, C, 16, 1, 1, gidx[0, kh, j])
+            assert np.abs(out[0, kh * G:(kh + 1) * G, j * C:(j + 1) * C] - ref).max() <= 2e-2
+            assert np.abs(lse[0, kh * G:(kh + 1) * G, j * C:(j + 1) * C] - rl).max() <= 2e-2
+
+
+def test_bf16_output_dtype():
+    w = W.Workload("bf16out", 1, 512, 4, 2, 64, "bf16", 1e4, topk_chunks=2, topk_groups=4, n_clusters=4)
+    q, k, v = W.generate(w, 2)
+    p, buf = parity.run_gpu(w, q, k, v, out_dtype=HGA_F32)
+    p2, buf2 = parity.run_gpu(w, q, k, v, out_dtype=HGA_BF16)
+    assert buf2.out.dtype == torch.bfloat16
+    assert (buf2.out.float() - buf.out).abs().max().item() <= 2.0 ** -6  # one bf16 rounding of |o| < 4
+
+
+def test_determinism_and_in_place_rope():
+    w = W.Workload("det", 1, 1024, 4, 2, 128, "bf16", 1e6, topk_chunks=4, topk_groups=12, n_clusters=4)
+    q, k, v = W.generate(w, 4)
+    p, a = parity.run_gpu(w, q, k, v)
+    _, b = parity.run_gpu(w, q, k, v)
+    for name in ("q_rot", "k_rot", "q_pooled", "chunk_sum", "group_sum", "chunk_idx", "group_idx", "out", "lse"):
+        assert torch.equal(getattr(a, name), getattr(b, name)), name
+    dq, dk, dv = parity.to_device(w, (q, k, v))
+    q2, pooled = hga.hga_rope(p, dq, x_rot=dq)  # in place
+    assert torch.equal(q2, a.q_rot) and torch.equal(pooled, a.q_pooled)
+
+
+def test_error_codes_on_device_calls():
+    w = W.Workload("err", 1, 512, 4, 2, 64, "bf16", 1e4)
+    p = hga.params_from_workload(w)
+    x = torch.zeros((1, 4, 512, 64), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(hga.HgaError) as e:
+        hga.hga_rope(p, x[:, :, :, :], x_rot=x, pooled=torch.zeros(17, device="cuda")[1:])  # misaligned pooled
+    assert e.value.code == 1
+    qp = torch.zeros((1, 2, 8, 64), device="cuda")
+    gs = torch.zeros((1, 2, 32, 64), device="cuda")
+    with pytest.raises(hga.HgaError) as e:
+        hga.hga_route(p, qp, qp, gs, workspace=torch.zeros(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == 3
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs 2..5 at FULL size, in the launch configuration bench.py times; sampled blocks
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,n_slices,n_blocks", [("c2", 3, 14), ("c3", 2, 14), ("c4", 2, 14), ("c5", 2, 12)])
+def test_full_size_sampled_parity(name, n_slices, n_blocks):
+    w = W.get(name)
+    q, k, v = W.generate(w, 0)
+    p, buf = parity.run_gpu(w, q, k, v)
+    rng = np.random.default_rng(1)
+    alls = _all_slices(w)
+    slices = [alls[i] for i in rng.choice(len(alls), size=n_slices, replace=False)]
+    blocks = _sample_blocks(w.n_blocks, n_blocks, 2)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, slices, blocks)
+    parity.assert_report(rep, w, len(slices) * len(blocks))
+    # property that holds at any size: every list is well formed and counts follow the budget rule
+    n_chunks = buf.n_chunks.cpu().numpy()
+    j = np.arange(w.n_blocks)
+    want = np.minimum(w.topk_chunks, np.maximum(0, j - max(w.n_local, 1) - w.n_sink))
+    assert np.array_equal(n_chunks, np.broadcast_to(want, n_chunks.shape))
+    assert np.array_equal(buf.n_groups.cpu().numpy(), np.minimum(w.topk_groups, 4 * n_chunks))
+    assert torch.isfinite(buf.out).all() and torch.isfinite(buf.lse).all()
