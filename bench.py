@@ -180,6 +180,27 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
+def reduce_max_over_ranks(x: float, dist, device) -> float:
+    """Timing rule: a multi-GPU number is the MAX over ranks (device-timed).  `dist` is torch.distributed or None."""
+    if dist is None:
+        return float(x)
+    import torch
+
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_tokens_per_s(world: int, tokens_per_rank: int, ms_per_step: float) -> float:
+    """Whole-job throughput of `world` independent replicas (weak scaling, no data-path collective)."""
+    return world * tokens_per_rank / (ms_per_step * 1e-3)
+
+
+def rank_seed(rank: int) -> int:
+    """Every rank runs its own replica of the workload on its own seeded inputs."""
+    return int(rank)
+
+
 def workload_config(w, args):
     return {"workload": f"{w.name}: B{w.batch} N{w.seq} Hq{w.n_q_heads}/Hkv{w.n_kv_heads} D{w.head_dim} {w.dtype} "
                         f"rope_base {w.rope_base:g}, C{w.chunk} g{w.group} F{w.n_sink} L{w.n_local} Kc{w.topk_chunks} "
@@ -213,7 +234,7 @@ def run_ours(args, w):
     hga.load_library()
     peaks, peak_src = load_peaks()
 
-    q, k, v = W.generate(w, rank)  # weak scaling: every rank runs its own replica of the workload (seed = rank)
+    q, k, v = W.generate(w, rank_seed(rank))  # weak scaling: every rank runs its own replica of the workload
     dt_io = torch.bfloat16 if w.dtype == "bf16" else torch.float32
     hq, hk, hv = (torch.from_numpy(a).to(dt_io).pin_memory() for a in (q, k, v))
     dq, dk, dv = (t.cuda(non_blocking=True) for t in (hq, hk, hv))
@@ -282,12 +303,9 @@ def run_ours(args, w):
         for s in range(4):
             stage_ms[s] += evs[i][s].elapsed_time(evs[i][s + 1])
     stage_ms /= K
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = reduce_max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / K
-    value = world * work["tokens"] / (ms_per_step * 1e-3)
+    value = job_tokens_per_s(world, work["tokens"], ms_per_step)
 
     # ---- e2e: host buffers through hga_host_prefill (H2D + S0..S4 + D2H inside the timed region) ---------------
     plan = hga.HostPlan(p)
@@ -301,11 +319,8 @@ def run_ours(args, w):
     for _ in range(Ke):
         plan.prefill(hq, hk, hv, out_host)   # returns after the plan's stream has drained
     e2e_s = (time.perf_counter() - t0) / Ke
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_value = world * work["tokens"] / e2e_s
+    e2e_s = reduce_max_over_ranks(e2e_s, dist, "cuda")
+    e2e_value = job_tokens_per_s(world, work["tokens"], e2e_s * 1e3)
     # cheap end-to-end sanity: the host path and the device path agree bit for bit
     same = bool(torch.equal(out_host.cuda(), buf.out))
     plan.close()
@@ -390,7 +405,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c5", help="c1..c5 (BASELINE.json configs[0..4]); default c5 = 64K Qwen3 shape")
-    ap.add_argument("--ref-blocks", type=int, default=24, help="query blocks in the oracle's bounded sample")
+    ap.add_argument("--ref-blocks", type=int, default=128, help="query blocks in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     import hga_workloads as W

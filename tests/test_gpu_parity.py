@@ -190,3 +190,35 @@ def test_full_size_sampled_parity(name, n_slices, n_blocks):
     assert np.array_equal(n_chunks, np.broadcast_to(want, n_chunks.shape))
     assert np.array_equal(buf.n_groups.cpu().numpy(), np.minimum(w.topk_groups, 4 * n_chunks))
     assert torch.isfinite(buf.out).all() and torch.isfinite(buf.lse).all()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs[4]: planted needle at 10 / 50 / 90 % depth must be in the routed set of the final block
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def c5_inputs():
+    w = W.get("c5")
+    return w, W.generate(w, 0)
+
+
+@pytest.mark.parametrize("depth", [0.10, 0.50, 0.90])
+def test_c5_needle_group_is_routed(c5_inputs, depth):
+    import needle
+
+    w, (q, k, v) = c5_inputs
+    kk = k.copy()
+    g_star = needle.plant(w, q, kk, depth)
+    p, buf = parity.run_gpu(w, q, kk, v)
+    last = w.n_blocks - 1
+    gidx = buf.group_idx[0, :, last].cpu().numpy()
+    cidx = buf.chunk_idx[0, :, last].cpu().numpy()
+    op = oracle.params_from_workload(w)
+    G = w.gqa
+    for kh in range(w.n_kv_heads):
+        r = oracle.prefill_slice(op, q[0, kh * G:(kh + 1) * G], kk[0, kh], v[0, kh], blocks=[last], attend=False,
+                                 want_k_rot=False)
+        assert g_star in r.group_idx[0]                      # the oracle routes it ...
+        assert g_star in gidx[kh] and g_star // 4 in cidx[kh]  # ... and so does the GPU
+    # and the whole final block (sets, scores, attention output) matches the oracle on the planted input
+    rep = parity.check_against_oracle(w, q, kk, v, p, buf, [(0, 0), (0, 3)], [last - 1, last])
+    parity.assert_report(rep, w, 4)

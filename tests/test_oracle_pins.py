@@ -453,3 +453,31 @@ def test_config1_tiny_cpu_checkable():
     pos = np.arange(1024)
     ref = sdpa_causal(rope_complex(q[0], pos[None].repeat(4, 0), 1e4), rope_complex(k[0, 0], pos, 1e4), v[0, 0])
     assert np.abs(r_all.out.transpose(1, 0, 2, 3).reshape(4, 1024, 64) - ref).max() < 1e-6
+
+
+def test_c5_needle_group_is_routed_by_the_oracle():
+    """BASELINE.json configs[4]: the planted 16-token needle group (cosine 0.9 with the final block's pooled rotated
+    query) must appear in the routed set of the final block, at 10 / 50 / 90 % depth.  Stand-in for PAPER.md:214-231."""
+    import needle
+
+    w = W.get("c5")
+    q, k, v = W.generate(w, 0)
+    op = oracle.params_from_workload(w)
+    G = w.gqa
+    for depth in needle.DEPTHS:
+        kk = k.copy()
+        g_star = needle.plant(w, q, kk, depth)
+        assert g_star == int(depth * w.n_groups_total) and (g_star * 16) // 64 not in (0, w.n_blocks - 2, w.n_blocks - 1)
+        # cosine of the planted rotated keys with the pooled rotated query of the final block is 0.9 (before rounding)
+        kh = 1
+        kr = oracle.rope(kk[0, kh, g_star * 16:(g_star + 1) * 16], g_star * 16, w.rope_base)
+        qb = oracle.pool_queries(oracle.rope(q[0, kh * G:(kh + 1) * G, -64:], w.seq - 64, w.rope_base), 64)[0]
+        cos = kr @ qb / (np.linalg.norm(kr, axis=1) * np.linalg.norm(qb))
+        assert np.all(np.abs(cos - 0.9) < 5e-3)
+        r = oracle.prefill_slice(op, q[0, kh * G:(kh + 1) * G], kk[0, kh], v[0, kh], blocks=[w.n_blocks - 1],
+                                 attend=False, want_k_rot=False)
+        assert g_star // 4 in r.chunk_idx[0] and g_star in r.group_idx[0]
+        # without the needle the same group is NOT routed (the planted signal, not chance, selects it)
+        r0 = oracle.prefill_slice(op, q[0, kh * G:(kh + 1) * G], k[0, kh], v[0, kh], blocks=[w.n_blocks - 1],
+                                  attend=False, want_k_rot=False)
+        assert g_star not in r0.group_idx[0]
