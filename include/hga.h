@@ -66,7 +66,10 @@ typedef enum { HGA_F32 = 0, HGA_BF16 = 1 } hga_dtype;
 typedef enum {
   HGA_ATTEND_AUTO = 0,    /* bf16 -> tcgen05/TMEM kernel, f32 -> SIMT fp32 kernel */
   HGA_ATTEND_SIMT = 1,    /* fp32 FMA kernel (any io_dtype): the 1e-4 path for fp32 inputs, and a cross-check */
-  HGA_ATTEND_TCGEN05 = 2  /* TMA gather + tcgen05.mma with TMEM accumulators (bf16 inputs only) */
+  HGA_ATTEND_TCGEN05 = 2, /* TMA gather + tcgen05.mma with TMEM accumulators (bf16 inputs only): the persistent
+                             kernel; falls back to HGA_ATTEND_TCGEN05_ITEM when the key list does not fit in
+                             shared memory beside the tiles */
+  HGA_ATTEND_TCGEN05_ITEM = 3 /* the same arithmetic, one (unit, tile pair) per CTA, no cross-item pipelining */
 } hga_attend_impl;
 
 /*

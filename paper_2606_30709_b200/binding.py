@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_PKG, "libhga.so")
 _lib = None
 
 HGA_F32, HGA_BF16 = 0, 1
-ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05 = 0, 1, 2
+ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM = 0, 1, 2, 3
 
 
 class HgaError(RuntimeError):

@@ -31,14 +31,14 @@ hga_status validate(const hga_params* p) {
   if (!(p->softmax_scale >= 0.0f) || !isfinite(p->softmax_scale)) return HGA_ERR_INVALID_ARG;
   if (p->io_dtype != HGA_F32 && p->io_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
   if (p->out_dtype != HGA_F32 && p->out_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
-  if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05) return HGA_ERR_INVALID_ARG;
+  if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05_ITEM) return HGA_ERR_INVALID_ARG;
   if (p->reserved != 0) return HGA_ERR_INVALID_ARG;
   if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
   // what the kernels implement
   if (p->chunk != kChunk) return HGA_ERR_UNSUPPORTED;
   if (p->group % 16) return HGA_ERR_UNSUPPORTED;
   if (p->head_dim != 64 && p->head_dim != 128) return HGA_ERR_UNSUPPORTED;
-  if (p->attend_impl == HGA_ATTEND_TCGEN05 && p->io_dtype != HGA_BF16) return HGA_ERR_UNSUPPORTED;
+  if (p->attend_impl >= HGA_ATTEND_TCGEN05 && p->io_dtype != HGA_BF16) return HGA_ERR_UNSUPPORTED;
   if ((long long)p->topk_groups * (p->group / 16) + (long long)(p->n_sink + p->n_local + 2) * 4 > 40000)
     return HGA_ERR_UNSUPPORTED;  // key list must fit in shared memory
   if ((long long)p->seq / p->chunk > 32768) return HGA_ERR_UNSUPPORTED;
@@ -155,7 +155,12 @@ hga_status hga_attend(const hga_params* p, const void* q_rot, const void* k_rot,
   if (!aligned16(q_rot) || !aligned16(k_rot) || !aligned16(v) || !aligned16(out)) return HGA_ERR_INVALID_ARG;
   int impl = p->attend_impl;
   if (impl == HGA_ATTEND_AUTO) impl = d.bf16_io ? HGA_ATTEND_TCGEN05 : HGA_ATTEND_SIMT;
-  if (impl == HGA_ATTEND_TCGEN05)
+  if (impl == HGA_ATTEND_TCGEN05) {
+    st = launch_attend_tc2(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
+    if (st != HGA_ERR_UNSUPPORTED) return st;
+    impl = HGA_ATTEND_TCGEN05_ITEM;
+  }
+  if (impl == HGA_ATTEND_TCGEN05_ITEM)
     return launch_attend_tc(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
   return launch_attend_simt(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
 }

@@ -1,0 +1,625 @@
+// S4, persistent tensor-core kernel for bf16 inputs (Eq. (1) PAPER.md:56 over the union set).
+//
+// One CTA per SM loops over work items; an item = one (batch, kv head, query block j) unit x two 128-row query
+// tiles (a tile = 2 query heads of the GQA group x 64 tokens).  Every role runs the same item sequence and the
+// roles are decoupled by mbarriers only, so the pipeline never drains between items: while the softmax
+// warpgroups finish item n, the producer already gathers item n+1's keys, the tensor pipe starts its first
+// Q K^T, and the epilogue warpgroup drains item n's output.
+//
+//   warps 0-3 / 4-7  softmax warpgroups (query tile 0 / 1), one thread per query row, ping-pong on the tensor pipe
+//   warps 8-11       epilogue: O_t / l -> swizzled staging tile -> TMA store
+//   warp 12          tcgen05.mma issuer (one thread):  S_t = Q_t K^T (SS),  O_t += P_t V (TS, P_t bf16 in TMEM)
+//   warp 13          TMA producer: gathers the K and V pieces of the key list (16 rows x 64 bf16 boxes, 128B swizzle)
+//   warp 14          key-list builder for the next item (double buffered)
+//
+// Key order inside an item: current chunk first (so the causal mask lives only in columns 0..63 of tile 0), then
+// sink chunks, routed groups, local chunks; only the last 128-key tile can be partial.
+// TMEM map (512 columns): S_t at t*128 (P_t overlays its first 64 columns), O_t at 256 + t*D.
+//
+// Softmax arithmetic: fp32, base-2 (scores scaled by scale*log2 e), running max refreshed lazily (only when it grows
+// by more than 2^8, which leaves the result mathematically unchanged), packed FFMA2/FADD2, FMNMX3 row max, and a
+// share of the exponentials evaluated on the FMA pipe (Cody-Waite + degree-3 polynomial, rel. error 7.5e-5, far
+// below the bf16 rounding of P) because MUFU.EX2 (16/clk/SM) would otherwise pace the 128x128 tiles.
+#include <cuda.h>
+#include <math_constants.h>
+
+#include "hga_common.cuh"
+#include "hga_tc_ptx.cuh"
+
+namespace hga {
+
+namespace {
+
+using namespace tc;
+
+constexpr int kThreads = 512;
+constexpr int kEpiWarp0 = 8;
+constexpr int kMmaWarp = 12;
+constexpr int kLoadWarp = 13;
+constexpr int kListWarp = 14;
+constexpr int kTileKeys = 128;  // keys per KV tile (8 pieces of 16)
+constexpr int kPPT = 8;         // pieces per tile
+constexpr float kRescaleThreshold = 8.0f;  // log2 units
+constexpr int kRegsSoftmax = 200, kRegsEpi = 64, kRegsCtl = 48;  // 2*128*200 + 128*64 + 128*48 = 65536
+
+// exp2 on the FMA pipe for pairs p with (p % kEmuPeriod) < kEmuCount
+constexpr int kEmuPeriod = 4;
+constexpr int kEmuCount = 1;
+
+struct Tc2Params {
+  int B, Hq, Hkv, N, n_b, G;
+  int F, L_eff, gs, Kg;
+  int n_mt;           // 128-row query tiles per unit = ceil(G/2)
+  int ctas_per_unit;  // ceil(n_mt/2)
+  int list_cap;       // pieces per list buffer
+  int n_items;
+  float scale_log2;   // softmax_scale * log2(e)
+  int out_bf16;
+};
+
+template <int D>
+struct Smem2 {
+  static constexpr int kHalves = D / 64;                   // 64-element (128-byte) column blocks
+  static constexpr int kHalfBytes = kTileKeys * 128;       // 128 rows x 128 B = 16 KB
+  static constexpr int kTileBytes = kHalves * kHalfBytes;  // Q tile / K tile / V tile
+  static constexpr int kStages = (D == 128) ? 2 : 4;
+  static constexpr int kQ = 0;
+  static constexpr int kK = kQ + 2 * kTileBytes;
+  static constexpr int kV = kK + kStages * kTileBytes;
+  static constexpr int kStage = kV + kStages * kTileBytes;  // epilogue staging: 4 warps x 4 KB
+  static constexpr int kBar = kStage + 4 * 4096;
+  // barrier ids
+  static constexpr int QFULL = 0, QEMPTY = 2, SFULL = 4, PFULL = 6, OFULL = 8, OEMPTY = 10, LFULL = 12, LEMPTY = 14,
+                       LISTFULL = 16, LISTEMPTY = 18, KFULL = 20, KEMPTY = KFULL + kStages, VFULL = KEMPTY + kStages,
+                       VEMPTY = VFULL + kStages, kNumBars = VEMPTY + kStages;
+  static constexpr int kMisc = kBar + 8 * kNumBars;  // tmem base (4 B), n_pieces[2]
+  static constexpr int kInvL = kMisc + 16;           // 2 tiles x 128 rows fp32
+  static constexpr int kList = kInvL + 2 * 128 * 4;  // 2 x list_cap ints
+};
+
+struct Item {
+  int b, kv, j, mt0, nt;
+};
+
+__device__ __forceinline__ Item decode_item(int it, const Tc2Params& prm) {
+  // heavy items first: j descending; the CTAs of one unit are adjacent so that their K/V gathers share L2 lines
+  const int per_j = prm.B * prm.Hkv * prm.ctas_per_unit;
+  Item r;
+  r.j = prm.n_b - 1 - it / per_j;
+  int rest = it % per_j;
+  const int cu = rest % prm.ctas_per_unit;
+  rest /= prm.ctas_per_unit;
+  r.kv = rest % prm.Hkv;
+  r.b = rest / prm.Hkv;
+  r.mt0 = cu * 2;
+  r.nt = min(2, prm.n_mt - r.mt0);
+  return r;
+}
+
+// exp2(x) for x <= ~8 evaluated without MUFU: n = round(x), r = x - n in [-0.5, 0.5], 2^r by a degree-3 polynomial
+// (weighted least squares on Chebyshev nodes, max rel. error 7.5e-5), exponent added in the integer domain.
+__device__ __forceinline__ void exp2_poly2(float x0, float x1, float& p0, float& p1) {
+  const float kMagic = 12582912.0f;  // 1.5 * 2^23: adding it rounds to the nearest integer in the low mantissa bits
+  x0 = fmaxf(x0, -125.0f);
+  x1 = fmaxf(x1, -125.0f);
+  const uint64_t x = pack2(x0, x1);
+  const uint64_t magic = pack2(kMagic, kMagic);
+  const uint64_t t = add2(x, magic);
+  const uint64_t nf = add2(t, pack2(-kMagic, -kMagic));
+  const uint64_t r = fma2(nf, pack2(-1.0f, -1.0f), x);
+  uint64_t p = fma2(pack2(0.0551716648042202f, 0.0551716648042202f), r, pack2(0.2426111251115799f, 0.2426111251115799f));
+  p = fma2(p, r, pack2(0.6932609677314758f, 0.6932609677314758f));
+  p = fma2(p, r, pack2(0.9999280571937561f, 0.9999280571937561f));
+  float t0, t1, q0, q1;
+  unpack2(t, t0, t1);
+  unpack2(p, q0, q1);
+  p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
+  p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                  const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
+                  const int32_t* __restrict__ group_idx, float* __restrict__ lse, const Tc2Params prm) {
+  using L = Smem2<D>;
+  extern __shared__ __align__(1024) unsigned char smem[];
+  const uint32_t sbase = smem_u32(smem);
+  auto BAR = [&](int i) { return sbase + (uint32_t)L::kBar + 8u * (uint32_t)i; };
+  volatile uint32_t* tmem_base_p = reinterpret_cast<volatile uint32_t*>(smem + L::kMisc);
+  volatile int* s_np = reinterpret_cast<volatile int*>(smem + L::kMisc + 4);  // [2]
+  float* s_invl = reinterpret_cast<float*>(smem + L::kInvL);                  // [2][128]
+  int* s_list = reinterpret_cast<int*>(smem + L::kList);                      // [2][list_cap]
+
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+
+  if (threadIdx.x == 0) {
+    if (sbase & 1023u) __trap();  // the 128B-swizzled tiles need a 1024-byte aligned base
+    for (int t = 0; t < 2; ++t) {
+      mbar_init(BAR(L::QFULL + t), 1);
+      mbar_init(BAR(L::QEMPTY + t), 1);
+      mbar_init(BAR(L::SFULL + t), 1);
+      mbar_init(BAR(L::PFULL + t), 4);
+      mbar_init(BAR(L::OFULL + t), 1);
+      mbar_init(BAR(L::OEMPTY + t), 4);
+      mbar_init(BAR(L::LFULL + t), 4);
+      mbar_init(BAR(L::LEMPTY + t), 4);
+      mbar_init(BAR(L::LISTFULL + t), 1);
+      mbar_init(BAR(L::LISTEMPTY + t), 10);  // producer + MMA + 8 softmax warps
+    }
+    for (int s = 0; s < L::kStages; ++s) {
+      mbar_init(BAR(L::KFULL + s), 1);
+      mbar_init(BAR(L::KEMPTY + s), 1);
+      mbar_init(BAR(L::VFULL + s), 1);
+      mbar_init(BAR(L::VEMPTY + s), 1);
+    }
+    fence_barrier_init();
+    fence_proxy_async();
+  }
+  if (warp == kMmaWarp) tmem_alloc(sbase + L::kMisc, 512);
+  if (warp == kLoadWarp && lane == 0) {
+    prefetch_tmap(&tmQ);
+    prefetch_tmap(&tmK);
+    prefetch_tmap(&tmV);
+  }
+  if (warp == kEpiWarp0 && lane == 0) prefetch_tmap(&tmO);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_base_p;
+
+  if (warp < 8) {
+    // ===================================== softmax warpgroups ===================================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
+    const int t = warp / 4;
+    const int row = (warp % 4) * 32 + lane;  // row of the 128-row tile == TMEM lane
+    const int r64 = row % 64;
+    const uint32_t lane_base = (uint32_t)((warp % 4) * 32) << 16;
+    const uint32_t s_addr = tmem + lane_base + (uint32_t)(t * 128);
+    const uint32_t o_addr = tmem + lane_base + (uint32_t)(256 + t * D);
+    const float sl2 = prm.scale_log2;
+    const uint64_t sl2x2 = pack2(sl2, sl2);
+    uint32_t s_cnt = 0;  // S_FULL completions consumed
+    uint32_t n_done = 0; // items this warpgroup has processed
+    int k = 0;
+    for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x, ++k) {
+      const Item im = decode_item(it, prm);
+      const int buf = k & 1;
+      mbar_wait(BAR(L::LISTFULL + buf), (uint32_t)(k >> 1) & 1u);
+      const int n_pieces = s_np[buf];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
+      if (t >= im.nt) continue;
+      const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
+      float m_run = -CUDART_INF_F;  // running reference max, raw logit units
+      float l_run = 0.f;
+      for (int i = 0; i < n_tiles; ++i) {
+        const int nk = min(kPPT, n_pieces - i * kPPT) * 16;  // valid key columns of this tile
+        mbar_wait(BAR(L::SFULL + t), s_cnt & 1u);
+        ++s_cnt;
+        tc_fence_after();
+        uint32_t sr[128];
+        tmem_ld32(s_addr + 0, sr + 0);
+        tmem_ld32(s_addr + 32, sr + 32);
+        tmem_ld32(s_addr + 64, sr + 64);
+        tmem_ld32(s_addr + 96, sr + 96);
+        tmem_wait_ld();
+        if (i == 0) {
+          // causal mask of the current chunk: key column c (< 64) is token j*64 + c
+#pragma unroll
+          for (int c = 1; c < 64; ++c)
+            if (c > r64) sr[c] = __float_as_uint(-CUDART_INF_F);
+        }
+        if (nk < kTileKeys) {
+#pragma unroll
+          for (int c = 16; c < 128; ++c)
+            if (c >= nk) sr[c] = __float_as_uint(-CUDART_INF_F);
+        }
+        float mx0 = max3(__uint_as_float(sr[0]), __uint_as_float(sr[1]), __uint_as_float(sr[2]));
+        float mx1 = max3(__uint_as_float(sr[3]), __uint_as_float(sr[4]), __uint_as_float(sr[5]));
+        float mx2 = max3(__uint_as_float(sr[6]), __uint_as_float(sr[7]), __uint_as_float(sr[8]));
+        float mx3 = max3(__uint_as_float(sr[9]), __uint_as_float(sr[10]), __uint_as_float(sr[11]));
+#pragma unroll
+        for (int c = 12; c < 124; c += 8) {
+          mx0 = max3(mx0, __uint_as_float(sr[c]), __uint_as_float(sr[c + 1]));
+          mx1 = max3(mx1, __uint_as_float(sr[c + 2]), __uint_as_float(sr[c + 3]));
+          mx2 = max3(mx2, __uint_as_float(sr[c + 4]), __uint_as_float(sr[c + 5]));
+          mx3 = max3(mx3, __uint_as_float(sr[c + 6]), __uint_as_float(sr[c + 7]));
+        }
+        mx0 = max3(mx0, __uint_as_float(sr[124]), __uint_as_float(sr[125]));
+        mx1 = max3(mx1, __uint_as_float(sr[126]), __uint_as_float(sr[127]));
+        const float m_new = fmaxf(m_run, fmaxf(max3(mx0, mx1, mx2), mx3));
+        const bool need = (m_new - m_run) * sl2 > kRescaleThreshold;  // first tile: +inf > 8
+        if (__any_sync(0xffffffffu, need)) {
+          float alpha = 1.f;
+          if (need) {
+            alpha = (m_run == -CUDART_INF_F) ? 0.f : fast_exp2((m_run - m_new) * sl2);
+            m_run = m_new;
+            l_run *= alpha;
+          }
+          if (i > 0) {
+            // O_t is quiescent here: S_FULL(i) was committed after PV(t, i-1)
+#pragma unroll
+            for (int c0 = 0; c0 < D; c0 += 32) {
+              uint32_t orr[32];
+              tmem_ld32(o_addr + c0, orr);
+              tmem_wait_ld();
+#pragma unroll
+              for (int c = 0; c < 32; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
+              tmem_st32(o_addr + c0, orr);
+            }
+          }
+        }
+        const float neg_m = -m_run * sl2;  // finite: the diagonal key of tile 0 is never masked
+        const uint64_t negm2 = pack2(neg_m, neg_m);
+        uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
+#pragma unroll
+        for (int c0 = 0; c0 < 128; c0 += 32) {
+          uint32_t pr[16];
+#pragma unroll
+          for (int c = 0; c < 16; ++c) {
+            const int pi = (c0 / 2 + c);  // pair index 0..63
+            const uint64_t x = fma2(pack2(__uint_as_float(sr[c0 + 2 * c]), __uint_as_float(sr[c0 + 2 * c + 1])), sl2x2, negm2);
+            float x0, x1, p0, p1;
+            unpack2(x, x0, x1);
+            if ((pi % kEmuPeriod) < kEmuCount) {
+              exp2_poly2(x0, x1, p0, p1);
+            } else {
+              p0 = fast_exp2(x0);
+              p1 = fast_exp2(x1);
+            }
+            pr[c] = cvt_bf16x2(p0, p1);  // low half = key 2c, high half = key 2c+1
+            if (c & 1) acc1 = add2(acc1, pack2(p0, p1));
+            else acc0 = add2(acc0, pack2(p0, p1));
+          }
+          tmem_st16(s_addr + (uint32_t)(c0 / 2), pr);  // P overlays S (already in registers)
+        }
+        float a0, a1;
+        unpack2(add2(acc0, acc1), a0, a1);
+        l_run += a0 + a1;
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(BAR(L::PFULL + t));
+      }
+      // ---- item done: hand 1/l to the epilogue warpgroup, write LSE ----------------------------------------------
+      mbar_wait(BAR(L::LEMPTY + t), (n_done & 1u) ^ 1u);
+      ++n_done;
+      s_invl[t * 128 + row] = 1.f / l_run;
+      const int head_in_group = (im.mt0 + t) * 2 + row / 64;
+      if (lse != nullptr && head_in_group < prm.G) {
+        const size_t orow = ((size_t)im.b * prm.Hq + (size_t)(im.kv * prm.G + head_in_group)) * prm.N + (size_t)im.j * kChunk + r64;
+        lse[orow] = (m_run * sl2 + log2f(l_run)) * 0.69314718055994530942f;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(BAR(L::LFULL + t));
+    }
+  } else if (warp < kMmaWarp) {
+    // ===================================== epilogue warpgroup ===================================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsEpi));
+    const int e = warp - kEpiWarp0;  // TMEM lanes 32e .. 32e+31
+    const uint32_t lane_base = (uint32_t)(e * 32) << 16;
+    const uint32_t stage = sbase + (uint32_t)L::kStage + (uint32_t)e * 4096u;
+    unsigned char* stage_p = smem + L::kStage + e * 4096;
+    const int colw = prm.out_bf16 ? 64 : 32;  // columns per 128-byte staging row
+    uint32_t o_cnt[2] = {0, 0};  // items drained per tile
+    for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x) {
+      const Item im = decode_item(it, prm);
+      for (int t = 0; t < im.nt; ++t) {
+        mbar_wait(BAR(L::OFULL + t), o_cnt[t] & 1u);
+        mbar_wait(BAR(L::LFULL + t), o_cnt[t] & 1u);
+        ++o_cnt[t];
+        tc_fence_after();
+        const float inv = s_invl[t * 128 + e * 32 + lane];
+        const int head_in_group = (im.mt0 + t) * 2 + e / 2;
+        const bool live = head_in_group < prm.G;
+        const int grow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk + (e % 2) * 32;
+        const uint32_t o_addr = tmem + lane_base + (uint32_t)(256 + t * D);
+        for (int c0 = 0; c0 < D; c0 += colw) {
+          uint32_t w[32];
+          if (prm.out_bf16) {
+            uint32_t orr[32];
+            tmem_ld32(o_addr + c0, orr);
+            tmem_wait_ld();
+#pragma unroll
+            for (int c = 0; c < 16; ++c)
+              w[c] = cvt_bf16x2(__uint_as_float(orr[2 * c]) * inv, __uint_as_float(orr[2 * c + 1]) * inv);
+            tmem_ld32(o_addr + c0 + 32, orr);
+            tmem_wait_ld();
+#pragma unroll
+            for (int c = 0; c < 16; ++c)
+              w[16 + c] = cvt_bf16x2(__uint_as_float(orr[2 * c]) * inv, __uint_as_float(orr[2 * c + 1]) * inv);
+          } else {
+            tmem_ld32(o_addr + c0, w);
+            tmem_wait_ld();
+#pragma unroll
+            for (int c = 0; c < 32; ++c) w[c] = __float_as_uint(__uint_as_float(w[c]) * inv);
+          }
+          if (live) {
+            if (lane == 0) bulk_wait_read0();  // the previous store has finished reading the staging tile
+            __syncwarp();
+#pragma unroll
+            for (int c = 0; c < 8; ++c)  // row `lane`, 16-byte chunk c at its 128B-swizzled position
+              *reinterpret_cast<uint4*>(stage_p + lane * 128 + ((c ^ (lane & 7)) << 4)) =
+                  make_uint4(w[4 * c], w[4 * c + 1], w[4 * c + 2], w[4 * c + 3]);
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_2d(&tmO, stage, c0, grow);
+              bulk_commit();
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(BAR(L::OEMPTY + t));
+          mbar_arrive(BAR(L::LEMPTY + t));
+        }
+      }
+    }
+    if (lane == 0) bulk_wait0();
+  } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsCtl));
+    if (warp == kListWarp) {
+      // ===================================== key-list builder ===================================================
+      const int ppc = kChunk / 16, ppg = prm.gs / 16;
+      int k = 0;
+      for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x, ++k) {
+        const Item im = decode_item(it, prm);
+        const int buf = k & 1;
+        mbar_wait(BAR(L::LISTEMPTY + buf), ((uint32_t)(k >> 1) & 1u) ^ 1u);
+        int* list = s_list + buf * prm.list_cap;
+        const int j = im.j;
+        const int n_sink = min(prm.F, j);
+        const int loc_lo = max(max(0, j - prm.L_eff), n_sink);  // local chunks not already in the sink window
+        const int n_loc = max(0, j - loc_lo);
+        int n = 0;
+        for (int i = lane; i < ppc; i += 32) list[i] = j * ppc + i;  // current chunk first
+        n += ppc;
+        for (int i = lane; i < n_sink * ppc; i += 32) list[n + i] = i;
+        n += n_sink * ppc;
+        // routed: closed earlier groups outside the sink/local windows (set union), compacted in list order so
+        // that the summation order of the softmax is the same on every run
+        if (group_idx != nullptr) {
+          const int32_t* gi = group_idx + (((size_t)im.b * prm.Hkv + im.kv) * prm.n_b + j) * prm.Kg;
+          for (int i0 = 0; i0 < prm.Kg; i0 += 32) {
+            const int i = i0 + lane;
+            const int g = (i < prm.Kg) ? __ldg(gi + i) : -1;
+            bool keep = false;
+            if (g >= 0) {
+              const int c = (g * prm.gs) / kChunk;
+              keep = (c < j) && !(c < n_sink) && !(c >= loc_lo);
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, keep);
+            if (keep) {
+              const int slot = n + __popc(m & ((1u << lane) - 1u)) * ppg;
+              for (int u = 0; u < ppg; ++u) list[slot + u] = g * ppg + u;
+            }
+            n += __popc(m) * ppg;
+          }
+        }
+        for (int i = lane; i < n_loc * ppc; i += 32) list[n + i] = loc_lo * ppc + i;
+        n += n_loc * ppc;
+        __syncwarp();
+        if (lane == 0) {
+          s_np[buf] = n;
+          mbar_arrive(BAR(L::LISTFULL + buf));
+        }
+      }
+    } else if (warp == kLoadWarp) {
+      // ===================================== TMA producer =======================================================
+      uint32_t fill = 0;  // K/V tiles issued so far (both rings advance together)
+      uint32_t qe_cnt[2] = {0, 0};  // Q tiles loaded per slot
+      int k = 0;
+      for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x, ++k) {
+        const Item im = decode_item(it, prm);
+        const int buf = k & 1;
+        mbar_wait(BAR(L::LISTFULL + buf), (uint32_t)(k >> 1) & 1u);
+        const int n_pieces = s_np[buf];
+        const int* list = s_list + buf * prm.list_cap;
+        const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
+        const int kv_row0 = (im.b * prm.Hkv + im.kv) * prm.N;  // row of token 0 in the flattened [B*Hkv*N, D] K/V
+        for (int i = 0; i < n_tiles; ++i, ++fill) {
+          const int s = (int)(fill % L::kStages);
+          const uint32_t ph = (fill / L::kStages) & 1u;
+          const int np = min(kPPT, n_pieces - i * kPPT);
+          const uint32_t bytes = (uint32_t)(np * 16 * D * 2);
+          const int pc = lane / L::kHalves, cb = lane % L::kHalves;
+          const bool active = lane < kPPT * L::kHalves && pc < np;
+          const int row = active ? kv_row0 + list[i * kPPT + pc] * 16 : 0;
+          const uint32_t off = (uint32_t)(s * L::kTileBytes + cb * L::kHalfBytes + pc * 16 * 128);
+          mbar_wait(BAR(L::KEMPTY + s), ph ^ 1u);
+          if (lane == 0) mbar_expect_tx(BAR(L::KFULL + s), bytes);
+          __syncwarp();
+          if (active) tma_load_2d(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s));
+          if (i == 0) {
+            // Q tiles of this item: (tile t, head-in-tile hh, column block cb) -> 64 rows x 64 columns
+            for (int t = 0; t < im.nt; ++t) {
+              mbar_wait(BAR(L::QEMPTY + t), (qe_cnt[t] & 1u) ^ 1u);
+              ++qe_cnt[t];
+              if (lane == 0) mbar_expect_tx(BAR(L::QFULL + t), (uint32_t)L::kTileBytes);
+              __syncwarp();
+              if (lane < 2 * L::kHalves) {
+                const int qcb = lane % L::kHalves, hh = lane / L::kHalves;
+                int head_in_group = (im.mt0 + t) * 2 + hh;
+                if (head_in_group >= prm.G) head_in_group = (im.mt0 + t) * 2;  // odd G: duplicate a live head, never stored
+                const int qrow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk;
+                tma_load_2d(sbase + L::kQ + t * L::kTileBytes + qcb * L::kHalfBytes + hh * 64 * 128, &tmQ, qcb * 64, qrow,
+                            BAR(L::QFULL + t));
+              }
+            }
+          }
+          mbar_wait(BAR(L::VEMPTY + s), ph ^ 1u);
+          if (lane == 0) mbar_expect_tx(BAR(L::VFULL + s), bytes);
+          __syncwarp();
+          if (active) tma_load_2d(sbase + L::kV + off, &tmV, cb * 64, row, BAR(L::VFULL + s));
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
+      }
+    } else if (warp == kMmaWarp) {
+      // ===================================== MMA issuer (one thread) ============================================
+      if (lane == 0) {
+        const uint32_t idesc_pv = umma_idesc(128, D, /*b_mn_major=*/true);
+        uint32_t q_cnt[2] = {0, 0};   // Q_FULL completions consumed per tile
+        uint32_t p_cnt[2] = {0, 0};   // P_FULL completions consumed per tile
+        uint32_t oe_cnt[2] = {0, 0};  // O_EMPTY waits per tile
+        auto issue_qk = [&](int t, int s, int nkeys) {
+          const uint32_t idesc = umma_idesc(128, nkeys, false);
+          const uint32_t qa = sbase + L::kQ + t * L::kTileBytes;
+          const uint32_t ka = sbase + L::kK + s * L::kTileBytes;
+#pragma unroll
+          for (int kk = 0; kk < D / 16; ++kk) {
+            const uint32_t o = (uint32_t)((kk / 4) * L::kHalfBytes + (kk % 4) * 32);
+            umma_ss(tmem + (uint32_t)(t * 128), umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc,
+                    kk > 0 ? 1u : 0u);
+          }
+        };
+        auto issue_pv = [&](int t, int s, int nkeys, bool first) {
+          const uint32_t va = sbase + L::kV + s * L::kTileBytes;
+          for (int kk = 0; kk < nkeys / 16; ++kk) {
+            // A: P_t columns [8kk, 8kk+8) (16 bf16 keys); B: V rows 16kk..16kk+15, MN-major, LBO = next 64 columns
+            umma_ts(tmem + (uint32_t)(256 + t * D), tmem + (uint32_t)(t * 128 + kk * 8),
+                    umma_desc(va + (uint32_t)(kk * 16 * 128), L::kHalfBytes, 1024), idesc_pv, (!first || kk > 0) ? 1u : 0u);
+          }
+        };
+        uint32_t step = 0;  // K/V tiles consumed so far: tile `step` lives in stage step % kStages
+        int k = 0;
+        int it = blockIdx.x;
+        int n_pieces = 0, nt = 0;
+        if (it < prm.n_items) {
+          mbar_wait(BAR(L::LISTFULL + 0), 0);
+          n_pieces = s_np[0];
+          nt = decode_item(it, prm).nt;
+          // first Q K^T of the first item
+          mbar_wait(BAR(L::KFULL + 0), 0);
+          for (int t = 0; t < nt; ++t) {
+            mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+            ++q_cnt[t];
+            tc_fence_after();
+            issue_qk(t, 0, min(kPPT, n_pieces) * 16);
+            umma_commit(BAR(L::SFULL + t));
+            if (n_pieces <= kPPT) umma_commit(BAR(L::QEMPTY + t));
+          }
+          umma_commit(BAR(L::KEMPTY + 0));
+        }
+        for (; it < prm.n_items; it += gridDim.x, ++k) {
+          const int buf = k & 1;
+          const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
+          const int it_next = it + gridDim.x;
+          const bool has_next = it_next < prm.n_items;
+          int n_pieces_next = 0, nt_next = 0;
+          for (int i = 0; i < n_tiles; ++i, ++step) {
+            const int vs = (int)(step % L::kStages);
+            const int ks = (int)((step + 1) % L::kStages);
+            const bool last = (i + 1 == n_tiles);
+            const bool more = !last || has_next;  // another Q K^T follows this tile's P V
+            int nkeys_next = 0, n_tiles_after = 0;
+            if (!last) {
+              nkeys_next = min(kPPT, n_pieces - (i + 1) * kPPT) * 16;
+              n_tiles_after = n_tiles - (i + 2);
+            } else if (has_next) {
+              mbar_wait(BAR(L::LISTFULL + (buf ^ 1)), (uint32_t)((k + 1) >> 1) & 1u);
+              n_pieces_next = s_np[buf ^ 1];
+              nt_next = decode_item(it_next, prm).nt;
+              nkeys_next = min(kPPT, n_pieces_next) * 16;
+              n_tiles_after = (n_pieces_next + kPPT - 1) / kPPT - 1;
+            }
+            const int nkeys = min(kPPT, n_pieces - i * kPPT) * 16;
+            mbar_wait(BAR(L::VFULL + vs), (step / L::kStages) & 1u);
+            if (more) mbar_wait(BAR(L::KFULL + ks), ((step + 1) / L::kStages) & 1u);
+            const int nt_qk = last ? nt_next : nt;
+            for (int t = 0; t < max(nt, nt_qk); ++t) {
+              if (t < nt) {
+                mbar_wait(BAR(L::PFULL + t), p_cnt[t] & 1u);
+                ++p_cnt[t];
+                if (i == 0) {
+                  // the epilogue has drained the previous item's O_t
+                  mbar_wait(BAR(L::OEMPTY + t), (oe_cnt[t] & 1u) ^ 1u);
+                  ++oe_cnt[t];
+                }
+                tc_fence_after();
+                issue_pv(t, vs, nkeys, i == 0);
+                if (last) umma_commit(BAR(L::OFULL + t));
+              }
+              if (more && t < nt_qk) {
+                if (last) {
+                  mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+                  ++q_cnt[t];
+                  tc_fence_after();
+                }
+                issue_qk(t, ks, nkeys_next);
+                umma_commit(BAR(L::SFULL + t));
+                if (n_tiles_after == 0) umma_commit(BAR(L::QEMPTY + t));  // that was the item's last Q K^T
+              }
+            }
+            umma_commit(BAR(L::VEMPTY + vs));
+            if (more) umma_commit(BAR(L::KEMPTY + ks));
+          }
+          mbar_arrive(BAR(L::LISTEMPTY + buf));
+          n_pieces = n_pieces_next;
+          nt = nt_next;
+        }
+      }
+      __syncwarp();
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kMmaWarp) {
+    tc_fence_after();
+    tmem_dealloc(tmem, 512);
+  }
+}
+
+template <int D>
+hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const void* v, const int32_t* gi, void* out,
+                        float* lse, cudaStream_t s) {
+  using L = Smem2<D>;
+  Tc2Params prm;
+  prm.B = d.B; prm.Hq = d.Hq; prm.Hkv = d.Hkv; prm.N = d.N; prm.n_b = d.n_b; prm.G = d.G;
+  prm.F = d.F; prm.L_eff = d.L_eff; prm.gs = d.gs; prm.Kg = d.Kg;
+  prm.n_mt = (d.G + 1) / 2;
+  prm.ctas_per_unit = (prm.n_mt + 1) / 2;
+  prm.list_cap = max_key_pieces(d.F, d.L_eff, d.gs, d.Kg);
+  prm.scale_log2 = d.scale * 1.4426950408889634f;
+  prm.out_bf16 = d.bf16_out ? 1 : 0;
+  const long long n_items = (long long)d.B * d.Hkv * d.n_b * prm.ctas_per_unit;
+  const size_t smem = (size_t)L::kList + 2 * sizeof(int) * (size_t)prm.list_cap;
+  if (smem > 227 * 1024 || n_items >= (1ll << 31)) return HGA_ERR_UNSUPPORTED;
+  if ((uint64_t)d.B * d.Hq * d.N >= (1ull << 31)) return HGA_ERR_UNSUPPORTED;
+  prm.n_items = (int)n_items;
+  CUtensorMap tmQ, tmK, tmV, tmO;
+  const uint64_t q_rows = (uint64_t)d.B * d.Hq * d.N, kv_rows = (uint64_t)d.B * d.Hkv * d.N;
+  bool ok = make_map_2d(&tmQ, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, q, q_rows, D, 64, 64) &&
+            make_map_2d(&tmK, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, k, kv_rows, D, 64, 16) &&
+            make_map_2d(&tmV, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, v, kv_rows, D, 64, 16);
+  ok = ok && (d.bf16_out ? make_map_2d(&tmO, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, out, q_rows, D, 64, 32)
+                         : make_map_2d(&tmO, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, out, q_rows, D, 32, 32));
+  if (!ok) return HGA_ERR_CUDA;
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    HGA_CUDA_OK(cudaGetDevice(&dev));
+    HGA_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  }
+  auto kern = attend_tc2_kernel<D>;
+  HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int grid = (int)(n_items < n_sm ? n_items : n_sm);
+  kern<<<grid, kThreads, smem, s>>>(tmQ, tmK, tmV, tmO, gi, lse, prm);
+  return launch_status();
+}
+
+}  // namespace
+
+// Returns HGA_ERR_UNSUPPORTED when the key list does not fit beside the tiles (the caller falls back to the
+// one-item-per-CTA kernel).
+hga_status launch_attend_tc2(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
+                             void* out, float* lse, cudaStream_t s) {
+  if (!d.bf16_io) return HGA_ERR_UNSUPPORTED;
+  return d.D == 128 ? launch_tc2_t<128>(d, q, k, v, group_idx, out, lse, s)
+                    : launch_tc2_t<64>(d, q, k, v, group_idx, out, lse, s);
+}
+
+}  // namespace hga

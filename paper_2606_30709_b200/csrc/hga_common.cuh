@@ -86,6 +86,8 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s);
 hga_status launch_attend_simt(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                               void* out, float* lse, cudaStream_t s);
+hga_status launch_attend_tc2(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
+                             void* out, float* lse, cudaStream_t s);
 hga_status launch_attend_tc(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                             void* out, float* lse, cudaStream_t s);
 

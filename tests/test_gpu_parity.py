@@ -11,7 +11,8 @@ import torch
 import hga_workloads as W
 import oracle
 import paper_2606_30709_b200 as hga
-from paper_2606_30709_b200.binding import ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, HGA_BF16, HGA_F32
+from paper_2606_30709_b200.binding import (ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM, HGA_BF16,
+                                             HGA_F32)
 
 import parity
 
@@ -75,7 +76,7 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05])
+@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM])
 @pytest.mark.parametrize("cfg", SMALL, ids=[c[0] for c in SMALL])
 def test_small_bf16_full_parity(cfg, impl):
     name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L = cfg
@@ -87,7 +88,7 @@ def test_small_bf16_full_parity(cfg, impl):
     parity.assert_report(rep, w, w.n_blocks * B * Hkv)
 
 
-@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05])
+@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM])
 def test_bf16_full_coverage_equals_dense(impl):
     """full chunk coverage must reproduce dense causal attention (bf16 bar: 2e-2)."""
     w = W.Workload("dense", 1, 1024, 8, 2, 128, "bf16", 1e6, topk_chunks=16, topk_groups=64, n_clusters=4)
@@ -102,7 +103,7 @@ def test_bf16_full_coverage_equals_dense(impl):
             assert np.abs(got[kh * 4:(kh + 1) * 4, j * 64:(j + 1) * 64] - ref).max() <= 2e-2
 
 
-@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05])
+@pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM])
 def test_attend_isolated_caller_supplied_lists(impl):
     """S4 alone: oracle-rotated Q/K and arbitrary (unsorted, padded, window-overlapping) group lists."""
     w = W.Workload("iso", 1, 1024, 4, 2, 128, "bf16", 1e6, topk_chunks=4, topk_groups=12, n_clusters=4)
