@@ -82,15 +82,17 @@ struct Item {
 };
 
 __device__ __forceinline__ Item decode_item(int it, const Tc2Params& prm) {
-  // heavy items first: j descending; the CTAs of one unit are adjacent so that their K/V gathers share L2 lines
-  const int per_j = prm.B * prm.Hkv * prm.ctas_per_unit;
+  // (batch, kv head) outermost: the K/V of one head (c5: 33.5 MB) then stays L2-resident while Q streams through,
+  // and the CTAs working at any moment share sink / routed / local lines.  Inside a head: j descending (longest
+  // lists first, the short early blocks fill the tail), the CTAs of one unit adjacent.
+  const int per_head = prm.n_b * prm.ctas_per_unit;
   Item r;
-  r.j = prm.n_b - 1 - it / per_j;
-  int rest = it % per_j;
-  const int cu = rest % prm.ctas_per_unit;
-  rest /= prm.ctas_per_unit;
-  r.kv = rest % prm.Hkv;
-  r.b = rest / prm.Hkv;
+  const int bk = it / per_head;
+  const int rem = it % per_head;
+  r.j = prm.n_b - 1 - rem / prm.ctas_per_unit;
+  const int cu = rem % prm.ctas_per_unit;
+  r.kv = bk % prm.Hkv;
+  r.b = bk / prm.Hkv;
   r.mt0 = cu * 2;
   r.nt = min(2, prm.n_mt - r.mt0);
   return r;
@@ -303,6 +305,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     unsigned char* stage_p = smem + L::kStage + e * 4096;
     const int colw = prm.out_bf16 ? 64 : 32;  // columns per 128-byte staging row
     uint32_t o_cnt[2] = {0, 0};  // items drained per tile
+    const uint64_t pol_o = policy_evict_first();
     for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x) {
       const Item im = decode_item(it, prm);
       for (int t = 0; t < im.nt; ++t) {
@@ -345,7 +348,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) {
-              tma_store_2d(&tmO, stage, c0, grow);
+              tma_store_2d_hint(&tmO, stage, c0, grow, pol_o);
               bulk_commit();
             }
           }
@@ -409,6 +412,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       }
     } else if (warp == kLoadWarp) {
       // ===================================== TMA producer =======================================================
+      const uint64_t pol_kv = policy_evict_last(), pol_q = policy_evict_first();
       uint32_t fill = 0;  // K/V tiles issued so far (both rings advance together)
       uint32_t qe_cnt[2] = {0, 0};  // Q tiles loaded per slot
       int k = 0;
@@ -432,7 +436,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           mbar_wait(BAR(L::KEMPTY + s), ph ^ 1u);
           if (lane == 0) mbar_expect_tx(BAR(L::KFULL + s), bytes);
           __syncwarp();
-          if (active) tma_load_2d(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s));
+          if (active) tma_load_2d_hint(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s), pol_kv);
           if (i == 0) {
             // Q tiles of this item: (tile t, head-in-tile hh, column block cb) -> 64 rows x 64 columns
             for (int t = 0; t < im.nt; ++t) {
@@ -445,122 +449,140 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                 int head_in_group = (im.mt0 + t) * 2 + hh;
                 if (head_in_group >= prm.G) head_in_group = (im.mt0 + t) * 2;  // odd G: duplicate a live head, never stored
                 const int qrow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk;
-                tma_load_2d(sbase + L::kQ + t * L::kTileBytes + qcb * L::kHalfBytes + hh * 64 * 128, &tmQ, qcb * 64, qrow,
-                            BAR(L::QFULL + t));
+                tma_load_2d_hint(sbase + L::kQ + t * L::kTileBytes + qcb * L::kHalfBytes + hh * 64 * 128, &tmQ, qcb * 64,
+                                 qrow, BAR(L::QFULL + t), pol_q);
               }
             }
           }
           mbar_wait(BAR(L::VEMPTY + s), ph ^ 1u);
           if (lane == 0) mbar_expect_tx(BAR(L::VFULL + s), bytes);
           __syncwarp();
-          if (active) tma_load_2d(sbase + L::kV + off, &tmV, cb * 64, row, BAR(L::VFULL + s));
+          if (active) tma_load_2d_hint(sbase + L::kV + off, &tmV, cb * 64, row, BAR(L::VFULL + s), pol_kv);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
       }
     } else if (warp == kMmaWarp) {
-      // ===================================== MMA issuer (one thread) ============================================
-      if (lane == 0) {
-        const uint32_t idesc_pv = umma_idesc(128, D, /*b_mn_major=*/true);
-        uint32_t q_cnt[2] = {0, 0};   // Q_FULL completions consumed per tile
-        uint32_t p_cnt[2] = {0, 0};   // P_FULL completions consumed per tile
-        uint32_t oe_cnt[2] = {0, 0};  // O_EMPTY waits per tile
-        auto issue_qk = [&](int t, int s, int nkeys) {
-          const uint32_t idesc = umma_idesc(128, nkeys, false);
-          const uint32_t qa = sbase + L::kQ + t * L::kTileBytes;
-          const uint32_t ka = sbase + L::kK + s * L::kTileBytes;
+      // ===================================== MMA issuer ==========================================================
+      // The whole warp runs the control flow convergently (so operands stay warp-uniform and ptxas needs no
+      // per-lane broadcast loops); only the tcgen05 instructions themselves are predicated on one elected lane.
+      const uint32_t ld = elect_one();
+      const uint32_t idesc_pv = umma_idesc(128, D, /*b_mn_major=*/true);
+      const uint32_t idesc_qk_full = umma_idesc(128, kTileKeys, false);
+      // descriptor high words are constant: SBO = 1024 B, version 1, SWIZZLE_128B
+      constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
+      constexpr uint32_t kLboK = (16u >> 4) << 16;                      // K-major operands (Q, K)
+      constexpr uint32_t kLboV = ((uint32_t)L::kHalfBytes >> 4) << 16;  // MN-major V: next 64 columns
+      uint32_t q_cnt0 = 0, q_cnt1 = 0;    // Q_FULL completions consumed per tile
+      uint32_t p_cnt0 = 0, p_cnt1 = 0;    // P_FULL completions consumed per tile
+      uint32_t oe_cnt0 = 0, oe_cnt1 = 0;  // O_EMPTY waits per tile
+      auto issue_qk = [&](int t, int s, int nkeys) {
+        const uint32_t idesc = nkeys == kTileKeys ? idesc_qk_full : umma_idesc(128, nkeys, false);
+        const uint32_t qa = ((sbase + L::kQ + t * L::kTileBytes) & 0x3FFFFu) >> 4;
+        const uint32_t ka = ((sbase + L::kK + s * L::kTileBytes) & 0x3FFFFu) >> 4;
+        const uint32_t d = tmem + (uint32_t)(t * 128);
 #pragma unroll
-          for (int kk = 0; kk < D / 16; ++kk) {
-            const uint32_t o = (uint32_t)((kk / 4) * L::kHalfBytes + (kk % 4) * 32);
-            umma_ss(tmem + (uint32_t)(t * 128), umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc,
-                    kk > 0 ? 1u : 0u);
-          }
-        };
-        auto issue_pv = [&](int t, int s, int nkeys, bool first) {
-          const uint32_t va = sbase + L::kV + s * L::kTileBytes;
-          for (int kk = 0; kk < nkeys / 16; ++kk) {
-            // A: P_t columns [8kk, 8kk+8) (16 bf16 keys); B: V rows 16kk..16kk+15, MN-major, LBO = next 64 columns
-            umma_ts(tmem + (uint32_t)(256 + t * D), tmem + (uint32_t)(t * 128 + kk * 8),
-                    umma_desc(va + (uint32_t)(kk * 16 * 128), L::kHalfBytes, 1024), idesc_pv, (!first || kk > 0) ? 1u : 0u);
-          }
-        };
-        uint32_t step = 0;  // K/V tiles consumed so far: tile `step` lives in stage step % kStages
-        int k = 0;
-        int it = blockIdx.x;
-        int n_pieces = 0, nt = 0;
-        if (it < prm.n_items) {
-          mbar_wait(BAR(L::LISTFULL + 0), 0);
-          n_pieces = s_np[0];
-          nt = decode_item(it, prm).nt;
-          // first Q K^T of the first item
-          mbar_wait(BAR(L::KFULL + 0), 0);
-          for (int t = 0; t < nt; ++t) {
-            mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
-            ++q_cnt[t];
-            tc_fence_after();
-            issue_qk(t, 0, min(kPPT, n_pieces) * 16);
-            umma_commit(BAR(L::SFULL + t));
-            if (n_pieces <= kPPT) umma_commit(BAR(L::QEMPTY + t));
-          }
-          umma_commit(BAR(L::KEMPTY + 0));
+        for (int kk = 0; kk < D / 16; ++kk) {
+          const uint32_t o = (uint32_t)((kk / 4) * L::kHalfBytes + (kk % 4) * 32) >> 4;
+          umma_ss_e(d, make_desc(qa + o + kLboK, kDescHi), make_desc(ka + o + kLboK, kDescHi), idesc, kk > 0 ? 1u : 0u, ld);
         }
-        for (; it < prm.n_items; it += gridDim.x, ++k) {
-          const int buf = k & 1;
-          const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
-          const int it_next = it + gridDim.x;
-          const bool has_next = it_next < prm.n_items;
-          int n_pieces_next = 0, nt_next = 0;
-          for (int i = 0; i < n_tiles; ++i, ++step) {
-            const int vs = (int)(step % L::kStages);
-            const int ks = (int)((step + 1) % L::kStages);
-            const bool last = (i + 1 == n_tiles);
-            const bool more = !last || has_next;  // another Q K^T follows this tile's P V
-            int nkeys_next = 0, n_tiles_after = 0;
-            if (!last) {
-              nkeys_next = min(kPPT, n_pieces - (i + 1) * kPPT) * 16;
-              n_tiles_after = n_tiles - (i + 2);
-            } else if (has_next) {
-              mbar_wait(BAR(L::LISTFULL + (buf ^ 1)), (uint32_t)((k + 1) >> 1) & 1u);
-              n_pieces_next = s_np[buf ^ 1];
-              nt_next = decode_item(it_next, prm).nt;
-              nkeys_next = min(kPPT, n_pieces_next) * 16;
-              n_tiles_after = (n_pieces_next + kPPT - 1) / kPPT - 1;
+      };
+      auto issue_pv = [&](int t, int s, int nkeys, bool first) {
+        const uint32_t va = ((sbase + L::kV + s * L::kTileBytes) & 0x3FFFFu) >> 4;
+        const uint32_t d = tmem + (uint32_t)(256 + t * D);
+        const uint32_t a = tmem + (uint32_t)(t * 128);
+        // A: P_t columns [8kk, 8kk+8) (16 bf16 keys); B: V rows 16kk..16kk+15, MN-major
+        if (nkeys == kTileKeys) {
+#pragma unroll
+          for (int kk = 0; kk < kPPT; ++kk)
+            umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(va + (uint32_t)(kk * 16 * 128 >> 4) + kLboV, kDescHi), idesc_pv,
+                      (!first || kk > 0) ? 1u : 0u, ld);
+        } else {
+          for (int kk = 0; kk < nkeys / 16; ++kk)
+            umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(va + (uint32_t)(kk * 16 * 128 >> 4) + kLboV, kDescHi), idesc_pv,
+                      (!first || kk > 0) ? 1u : 0u, ld);
+        }
+      };
+      uint32_t step = 0;  // K/V tiles consumed so far: tile `step` lives in stage step % kStages
+      int k = 0;
+      int it = blockIdx.x;
+      int n_pieces = 0, nt = 0;
+      if (it < prm.n_items) {
+        mbar_wait(BAR(L::LISTFULL + 0), 0);
+        n_pieces = s_np[0];
+        nt = decode_item(it, prm).nt;
+        // first Q K^T of the first item
+        mbar_wait(BAR(L::KFULL + 0), 0);
+        for (int t = 0; t < nt; ++t) {
+          mbar_wait(BAR(L::QFULL + t), 0);
+          if (t == 0) ++q_cnt0; else ++q_cnt1;
+          tc_fence_after();
+          issue_qk(t, 0, min(kPPT, n_pieces) * 16);
+          umma_commit_e(BAR(L::SFULL + t), ld);
+          if (n_pieces <= kPPT) umma_commit_e(BAR(L::QEMPTY + t), ld);
+        }
+        umma_commit_e(BAR(L::KEMPTY + 0), ld);
+      }
+      for (; it < prm.n_items; it += gridDim.x, ++k) {
+        const int buf = k & 1;
+        const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
+        const int it_next = it + gridDim.x;
+        const bool has_next = it_next < prm.n_items;
+        int n_pieces_next = 0, nt_next = 0;
+        for (int i = 0; i < n_tiles; ++i, ++step) {
+          const int vs = (int)(step % L::kStages);
+          const int ks = (int)((step + 1) % L::kStages);
+          const bool last = (i + 1 == n_tiles);
+          const bool more = !last || has_next;  // another Q K^T follows this tile's P V
+          int nkeys_next = 0, n_tiles_after = 0;
+          if (!last) {
+            nkeys_next = min(kPPT, n_pieces - (i + 1) * kPPT) * 16;
+            n_tiles_after = n_tiles - (i + 2);
+          } else if (has_next) {
+            mbar_wait(BAR(L::LISTFULL + (buf ^ 1)), (uint32_t)((k + 1) >> 1) & 1u);
+            n_pieces_next = s_np[buf ^ 1];
+            nt_next = decode_item(it_next, prm).nt;
+            nkeys_next = min(kPPT, n_pieces_next) * 16;
+            n_tiles_after = (n_pieces_next + kPPT - 1) / kPPT - 1;
+          }
+          const int nkeys = min(kPPT, n_pieces - i * kPPT) * 16;
+          mbar_wait(BAR(L::VFULL + vs), (step / L::kStages) & 1u);
+          if (more) mbar_wait(BAR(L::KFULL + ks), ((step + 1) / L::kStages) & 1u);
+          const int nt_qk = last ? nt_next : nt;
+#pragma unroll
+          for (int t = 0; t < 2; ++t) {
+            uint32_t& p_cnt = t == 0 ? p_cnt0 : p_cnt1;
+            uint32_t& oe_cnt = t == 0 ? oe_cnt0 : oe_cnt1;
+            uint32_t& q_cnt = t == 0 ? q_cnt0 : q_cnt1;
+            if (t < nt) {
+              mbar_wait(BAR(L::PFULL + t), p_cnt & 1u);
+              ++p_cnt;
+              if (i == 0) {
+                // the epilogue has drained the previous item's O_t
+                mbar_wait(BAR(L::OEMPTY + t), (oe_cnt & 1u) ^ 1u);
+                ++oe_cnt;
+              }
+              tc_fence_after();
+              issue_pv(t, vs, nkeys, i == 0);
+              if (last) umma_commit_e(BAR(L::OFULL + t), ld);
             }
-            const int nkeys = min(kPPT, n_pieces - i * kPPT) * 16;
-            mbar_wait(BAR(L::VFULL + vs), (step / L::kStages) & 1u);
-            if (more) mbar_wait(BAR(L::KFULL + ks), ((step + 1) / L::kStages) & 1u);
-            const int nt_qk = last ? nt_next : nt;
-            for (int t = 0; t < max(nt, nt_qk); ++t) {
-              if (t < nt) {
-                mbar_wait(BAR(L::PFULL + t), p_cnt[t] & 1u);
-                ++p_cnt[t];
-                if (i == 0) {
-                  // the epilogue has drained the previous item's O_t
-                  mbar_wait(BAR(L::OEMPTY + t), (oe_cnt[t] & 1u) ^ 1u);
-                  ++oe_cnt[t];
-                }
+            if (more && t < nt_qk) {
+              if (last) {
+                mbar_wait(BAR(L::QFULL + t), q_cnt & 1u);
+                ++q_cnt;
                 tc_fence_after();
-                issue_pv(t, vs, nkeys, i == 0);
-                if (last) umma_commit(BAR(L::OFULL + t));
               }
-              if (more && t < nt_qk) {
-                if (last) {
-                  mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
-                  ++q_cnt[t];
-                  tc_fence_after();
-                }
-                issue_qk(t, ks, nkeys_next);
-                umma_commit(BAR(L::SFULL + t));
-                if (n_tiles_after == 0) umma_commit(BAR(L::QEMPTY + t));  // that was the item's last Q K^T
-              }
+              issue_qk(t, ks, nkeys_next);
+              umma_commit_e(BAR(L::SFULL + t), ld);
+              if (n_tiles_after == 0) umma_commit_e(BAR(L::QEMPTY + t), ld);  // that was the item's last Q K^T
             }
-            umma_commit(BAR(L::VEMPTY + vs));
-            if (more) umma_commit(BAR(L::KEMPTY + ks));
           }
-          mbar_arrive(BAR(L::LISTEMPTY + buf));
-          n_pieces = n_pieces_next;
-          nt = nt_next;
+          umma_commit_e(BAR(L::VEMPTY + vs), ld);
+          if (more) umma_commit_e(BAR(L::KEMPTY + ks), ld);
         }
+        if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
+        n_pieces = n_pieces_next;
+        nt = nt_next;
       }
       __syncwarp();
     }
