@@ -167,10 +167,17 @@ hga_status hga_attend(const hga_params* p, const void* q_rot, const void* k_rot,
 
 hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) {
   if (!b) return HGA_ERR_INVALID_ARG;
-  hga_status st = hga_rope(p, b->q_raw, p ? p->n_q_heads : 0, b->q_rot, b->q_pooled, stream);
+  Derived d;
+  RopeFreq f;
+  hga_status st = derive(p, &d, &f);
   if (st != HGA_OK) return st;
-  if (!b->q_pooled || !b->k_rot || !b->chunk_sum) return HGA_ERR_INVALID_ARG;
-  st = hga_build_summaries(p, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum, stream);
+  if (!b->q_raw || !b->q_rot || !b->k_raw || !b->q_pooled || !b->k_rot || !b->chunk_sum) return HGA_ERR_INVALID_ARG;
+  if (!aligned16(b->q_raw) || !aligned16(b->q_rot) || !aligned16(b->q_pooled) || !aligned16(b->k_raw) ||
+      !aligned16(b->k_rot) || !aligned16(b->chunk_sum) || !aligned16(b->group_sum))
+    return HGA_ERR_INVALID_ARG;
+  // S0 + S1 in one launch: the K tiles and Q tiles of a (batch, chunk) row share the position tables
+  st = launch_rope_summaries(d, f, b->q_raw, b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum,
+                             (cudaStream_t)stream);
   if (st != HGA_OK) return st;
   st = hga_route(p, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
                  b->group_score, b->n_groups, b->workspace, b->workspace_bytes, stream);

@@ -81,6 +81,8 @@ hga_status launch_rope(const Derived& d, const RopeFreq& f, const void* x_raw, i
                        cudaStream_t s);
 hga_status launch_summaries(const Derived& d, const RopeFreq& f, const void* k_raw, void* k_rot, float* chunk_sum,
                             float* group_sum, cudaStream_t s);
+hga_status launch_rope_summaries(const Derived& d, const RopeFreq& f, const void* q_raw, void* q_rot, float* pooled,
+                                 const void* k_raw, void* k_rot, float* chunk_sum, float* group_sum, cudaStream_t s);
 hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
                         int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s);

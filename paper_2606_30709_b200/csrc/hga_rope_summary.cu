@@ -1,21 +1,36 @@
 // S0 (RoPE on Q + pooled block query) and S1 (RoPE on K + mixed-RoPE chunk/group summaries).
-// Both are one pass over their tensor: HBM-bound, 16-byte vector loads/stores, one CTA per 64-token chunk and a
-// few heads.  PAPER.md:62 (RoPE), 80-89 (summaries), 33/45/97 (chunk-shared per-KV-head routing query).
+// PAPER.md:62 (RoPE), 80-89 (summaries), 33/45/97 (chunk-shared per-KV-head routing query).
+//
+// One persistent, HBM-bound streaming kernel serves both stages (and both at once for hga_prefill):
+//   * a tile = the 64 tokens x D elements of one (batch, head, chunk) -- contiguous in memory, 8..32 KB;
+//   * every CTA owns a contiguous range of tiles, ordered (batch, chunk j) outermost; a consumer thread owns one
+//     (token, 8 RoPE pairs) item of every tile, keeps its (cos, sin) in registers and recomputes them only when j
+//     changes;
+//   * a producer warp streams tiles global -> shared through a ring of bulk async copies (cp.async.bulk + mbarrier
+//     complete_tx, full/empty barriers), so the bytes in flight per SM are set by the ring depth (128 KB), not by
+//     registers or occupancy; consumers pull their 32 bytes into registers, release the stage at once, rotate and
+//     write the result with 16-byte coalesced stores;
+//   * a row (batch, j) holds Hkv K tiles followed by Hq Q tiles; a Q "unit" is the G heads of one KV group, whose
+//     rotated values are pooled into the block's routing query; a K tile also yields its summaries.
 //
 // Numerics: the angle p*theta_i is reduced in fp64 (revolutions -> fractional part), the reduced angle is split
 // into an fp32 head and tail, sincosf() is taken on the head and corrected to first order with the tail, so
-// cos/sin carry ~1 ulp(fp32) error at any position.  The rotation is fp32 FMA; every mean is accumulated in fp64
-// from the un-rounded fp32 values and rounded once to float; the rotated tensor is rounded once to io_dtype.
+// cos/sin carry ~1 ulp(fp32) error at any position.  The rotation is fp32 FMA.  Means are taken from the un-rounded
+// fp32 values: per-thread / per-warp partial sums (at most 16 terms) in fp32 in a fixed order, combined in fp64
+// and rounded once to float; the rotated tensor is rounded once (RNE) to io_dtype.
 #include "hga_common.cuh"
+#include "hga_tc_ptx.cuh"
 
 namespace hga {
 
 namespace {
 
-constexpr int kThreads = 256;
+using namespace tc;
+
+constexpr int kMaxGpc = kChunk / 16;
 
 __device__ __forceinline__ double reduced_angle(double pos, double turns) {
-  double u = pos * turns;  // revolutions
+  double u = pos * turns;   // revolutions
   double fr = u - rint(u);  // [-0.5, 0.5]
   return fr * kTwoPi;
 }
@@ -29,285 +44,354 @@ __device__ __forceinline__ float2 cos_sin_f32(double pos, double turns) {
   return make_float2(fmaf(-sh, al, ch), fmaf(ch, al, sh));
 }
 
-// cs[t * half + i] = (cos, sin)((pos_first + t) * theta_i) for the chunk's 64 tokens.
-__device__ __forceinline__ void fill_table(float2* cs, const RopeFreq& f, int half, long long pos_first) {
-  for (int idx = threadIdx.x; idx < kChunk * half; idx += blockDim.x) {
-    int t = idx / half, i = idx - t * half;
-    cs[idx] = cos_sin_f32((double)(pos_first + t), f.turns[i]);
-  }
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
 }
 
-// ----------------------------------------------------------------------------------------------------------------
-// S0: x_rot = RoPE(x_raw); pooled = mean over (chunk tokens, heads of the pool group) of the rotated vectors.
-// grid (n_b, n_heads / heads_per_cta, B); heads_per_cta is a multiple of pool_heads.
-// ----------------------------------------------------------------------------------------------------------------
-template <typename T, int D>
-__global__ void __launch_bounds__(kThreads) rope_pool_kernel(const __grid_constant__ RopeFreq f,
-                                                             const T* x_raw, T* x_rot,  // may alias (in-place RoPE)
-                                                            
-                                                             float* __restrict__ pooled, int n_heads, int N, int n_b,
-                                                             int heads_per_cta, int pool_heads, long long pos0) {
-  constexpr int half = D / 2;
-  constexpr int OCT = D / 16;               // threads per token (8 pairs each)
-  constexpr int TOK_PER_PASS = kThreads / OCT;
-  constexpr int PASSES = kChunk / TOK_PER_PASS;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2* cs = reinterpret_cast<float2*>(smem_raw);                              // [64][half]
-  double* red = reinterpret_cast<double*>(smem_raw + sizeof(float2) * kChunk * half);  // [TOK_PER_PASS][D]
+struct RsParams {
+  const void* q_raw;
+  void* q_rot;
+  float* pooled;  // nullable
+  const void* k_raw;
+  void* k_rot;       // nullable: skip the store
+  float* chunk_sum;  // nullable
+  float* group_sum;  // nullable
+  int N, n_b;
+  int HQ, PG;  // heads of the "Q" tensor (0: none), heads pooled together (a Q unit)
+  int HK;      // heads of the "K" tensor (0: none)
+  int gs, gpc, n_hi_c, n_hi_g;
+  int tpr;     // tiles per row = HK + HQ
+  long long pos0;
+  long long total_tiles;  // rows * tpr
+};
 
-  const int j = blockIdx.x, b = blockIdx.z;
-  const int head0 = blockIdx.y * heads_per_cta;
-  fill_table(cs, f, half, pos0 + (long long)j * kChunk);
-  __syncthreads();
-
-  const int oct = threadIdx.x % OCT, slot = threadIdx.x / OCT;
-  const int i0 = oct * 8;
-  double acc[16];
-#pragma unroll
-  for (int u = 0; u < 16; ++u) acc[u] = 0.0;
-
-  for (int hh = 0; hh < heads_per_cta; ++hh) {
-    const int h = head0 + hh;
-    const size_t row0 = ((size_t)b * n_heads + h) * N + (size_t)j * kChunk;
-#pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps) {
-      const int t = ps * TOK_PER_PASS + slot;
-      const T* src = x_raw + (row0 + t) * D;
-      float a[8], bb[8], ra[8], rb[8];
-      Io<T>::load8(src + i0, a);
-      Io<T>::load8(src + half + i0, bb);
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        float2 c = cs[t * half + i0 + u];
-        ra[u] = fmaf(a[u], c.x, -(bb[u] * c.y));
-        rb[u] = fmaf(bb[u], c.x, a[u] * c.y);
-        acc[u] += (double)ra[u];
-        acc[8 + u] += (double)rb[u];
-      }
-      T* dst = x_rot + (row0 + t) * D;
-      Io<T>::store8(dst + i0, ra);
-      Io<T>::store8(dst + half + i0, rb);
-    }
-    if (pooled != nullptr && (hh + 1) % pool_heads == 0) {
-      // cross-thread reduction over the TOK_PER_PASS token slots, fixed order -> deterministic
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        red[slot * D + i0 + u] = acc[u];
-        red[slot * D + half + i0 + u] = acc[8 + u];
-        acc[u] = 0.0;
-        acc[8 + u] = 0.0;
-      }
-      __syncthreads();
-      if (threadIdx.x < D) {
-        double s = 0.0;
-        for (int q = 0; q < TOK_PER_PASS; ++q) s += red[q * D + threadIdx.x];
-        const int pg = h / pool_heads;  // pool group index == kv head
-        const int n_pg = n_heads / pool_heads;
-        pooled[(((size_t)b * n_pg + pg) * n_b + j) * D + threadIdx.x] = (float)(s / (double)(pool_heads * kChunk));
-      }
-      __syncthreads();
-    }
-  }
+// First tile of CTA `c` when `total` tiles are split over `n` CTAs at unit boundaries (a K tile, or PG Q tiles).
+__device__ __forceinline__ long long range_start(long long c, long long n, const RsParams& p) {
+  if (c >= n) return p.total_tiles;
+  const long long raw = c * p.total_tiles / n;
+  const long long row = raw / p.tpr;
+  int r = (int)(raw % p.tpr);
+  if (r > p.HK) r = p.HK + (r - p.HK + p.PG - 1) / p.PG * p.PG;
+  return row * p.tpr + r;
 }
 
-// ----------------------------------------------------------------------------------------------------------------
-// S1: k_rot = RoPE(k_raw); chunk and group summaries by the mixed rule.
-// grid (n_b, Hkv / heads_per_cta, B)
-// ----------------------------------------------------------------------------------------------------------------
 template <typename T, int D>
-__global__ void __launch_bounds__(kThreads) summaries_kernel(const __grid_constant__ RopeFreq f,
-                                                             const T* k_raw, T* k_rot,  // may alias (in-place RoPE)
-                                                            
-                                                             float* __restrict__ chunk_sum, float* __restrict__ group_sum,
-                                                             int Hkv, int N, int n_b, int heads_per_cta, int gs,
-                                                             int n_hi_c, int n_hi_g, long long pos0) {
-  constexpr int half = D / 2;
-  constexpr int OCT = D / 16;
-  constexpr int TOK_PER_PASS = kThreads / OCT;
-  constexpr int PASSES = kChunk / TOK_PER_PASS;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2* cs = reinterpret_cast<float2*>(smem_raw);                    // [64][half]
-  float* rot_s = reinterpret_cast<float*>(cs + kChunk * half);         // [64][D] rotated keys (fp32, un-rounded)
-  float* raw_s = rot_s + kChunk * D;                                   // [64][D] raw keys
-  double2* mid_g = reinterpret_cast<double2*>(raw_s + kChunk * D);     // [gpc][half] (cos, sin) at group middles
-  double2* mid_c = mid_g + (kChunk / 16) * half;                       // [half]      (cos, sin) at the chunk middle
-  double* dsum = reinterpret_cast<double*>(mid_c + half);              // [gpc][4][half]
+struct RsCfg {
+  static constexpr int kHalf = D / 2;
+  static constexpr int kOct = D / 16;                // threads per token (8 pairs each)
+  static constexpr int kConsumers = kChunk * kOct;   // one (token, 8 pairs) item per consumer thread
+  static constexpr int kCWarps = kConsumers / 32;
+  static constexpr int kThreads = kConsumers + 32;   // + the producer warp
+  static constexpr int kTpw = 32 / kOct;             // tokens per consumer warp
+  static constexpr int kCtasPerSm = (D == 128) ? 1 : 2;
+  static constexpr int kTileBytes = kChunk * D * (int)sizeof(T);
+  // shared memory map: fixed part first, the tile ring after it
+  static constexpr int kPart = 0;                                        // [2][kCWarps][2][D] float
+  static constexpr int kMid = kPart + 2 * kCWarps * 2 * D * 4;           // [2][kMaxGpc + 1][kHalf] double2
+  static constexpr int kTurns = kMid + 2 * (kMaxGpc + 1) * kHalf * 16;   // [kHalf] double
+  static constexpr int kBar = kTurns + kHalf * 8;                        // full[8], empty[8]
+  static constexpr int kTiles = (kBar + 16 * 8 + 127) / 128 * 128;
+  static constexpr int kBudget = (kCtasPerSm == 1 ? 200 : 100) * 1024;
+  static constexpr int kStagesRaw = (kBudget - kTiles) / kTileBytes;
+  static constexpr int kStages = kStagesRaw > 8 ? 8 : kStagesRaw;
+  static constexpr int kBytes = kTiles + kStages * kTileBytes;
+  static_assert(kStages >= 2, "ring too shallow");
+};
 
-  const int j = blockIdx.x, b = blockIdx.z;
-  const int head0 = blockIdx.y * heads_per_cta;
-  const int gpc = kChunk / gs;
-  const long long pos_first = pos0 + (long long)j * kChunk;
-  fill_table(cs, f, half, pos_first);
-  // middle positions (reading R2: start + (S-1)/2), full fp64 sincos -- once per CTA
-  for (int idx = threadIdx.x; idx < (gpc + 1) * half; idx += blockDim.x) {
-    int g = idx / half, i = idx - g * half;
-    double pm = (g < gpc) ? (double)pos_first + (double)(g * gs) + 0.5 * (double)(gs - 1)
-                          : (double)pos_first + 0.5 * (double)(kChunk - 1);
-    double s, c;
-    sincos(reduced_angle(pm, f.turns[i]), &s, &c);
-    if (g < gpc) mid_g[g * half + i] = make_double2(c, s);
-    else mid_c[i] = make_double2(c, s);
+__device__ __forceinline__ void consumer_sync(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
+
+template <typename T, int D>
+__global__ void __launch_bounds__(RsCfg<T, D>::kThreads, RsCfg<T, D>::kCtasPerSm)
+rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ RsParams p) {
+  using C = RsCfg<T, D>;
+  constexpr int half = C::kHalf, OCT = C::kOct, S = C::kStages, NW = C::kCWarps;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const uint32_t sbase = smem_u32(smem);
+  float* part_base = reinterpret_cast<float*>(smem + C::kPart);
+  double2* mid_base = reinterpret_cast<double2*>(smem + C::kMid);
+  double* s_turns = reinterpret_cast<double*>(smem + C::kTurns);
+  auto FULL = [&](int s) { return sbase + (uint32_t)C::kBar + 8u * (uint32_t)s; };
+  auto EMPTY = [&](int s) { return sbase + (uint32_t)C::kBar + 64u + 8u * (uint32_t)s; };
+
+  const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
+
+  const long long t0 = range_start(blockIdx.x, gridDim.x, p);
+  const long long t1 = range_start((long long)blockIdx.x + 1, gridDim.x, p);
+  const int nt = (int)(t1 - t0);
+
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(FULL(s), 1);
+      mbar_init(EMPTY(s), NW);
+    }
+    fence_barrier_init();
+    fence_proxy_async();
   }
+  for (int i = tid; i < half; i += C::kThreads) s_turns[i] = f.turns[i];
   __syncthreads();
 
-  const int oct = threadIdx.x % OCT, slot = threadIdx.x / OCT;
-  const int i0 = oct * 8;
-  // phase-B role: thread (g, i) sums group g, pair i
-  const int bg = threadIdx.x / half, bi = threadIdx.x % half;
-  const bool b_active = bg < gpc;
+  // position of the CTA's first tile; every role advances (b, j, r) incrementally
+  long long row0 = t0 / p.tpr;
+  int r = (int)(t0 % p.tpr);
+  int b = (int)(row0 / p.n_b), j = (int)(row0 % p.n_b);
 
-  for (int hh = 0; hh < heads_per_cta; ++hh) {
-    const int h = head0 + hh;
-    const size_t row0 = ((size_t)b * Hkv + h) * N + (size_t)j * kChunk;
-    // phase A: rotate, store, stage rotated + raw values in shared memory
-#pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps) {
-      const int t = ps * TOK_PER_PASS + slot;
-      const T* src = k_raw + (row0 + t) * D;
-      float a[8], bb[8], ra[8], rb[8];
-      Io<T>::load8(src + i0, a);
-      Io<T>::load8(src + half + i0, bb);
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        float2 c = cs[t * half + i0 + u];
-        ra[u] = fmaf(a[u], c.x, -(bb[u] * c.y));
-        rb[u] = fmaf(bb[u], c.x, a[u] * c.y);
+  if (warp == NW) {
+    // ===================================== producer: bulk loads into the ring ===================================
+    if (lane == 0) {
+      for (int k = 0; k < nt; ++k) {
+        const int s = k % S;
+        if (k >= S) mbar_wait(EMPTY(s), (uint32_t)(k / S - 1) & 1u);
+        const unsigned char* src;
+        if (r < p.HK) src = (const unsigned char*)p.k_raw + (((size_t)b * p.HK + r) * p.N + (size_t)j * kChunk) * D * sizeof(T);
+        else src = (const unsigned char*)p.q_raw + (((size_t)b * p.HQ + (r - p.HK)) * p.N + (size_t)j * kChunk) * D * sizeof(T);
+        mbar_expect_tx(FULL(s), (uint32_t)C::kTileBytes);
+        bulk_load(sbase + C::kTiles + s * C::kTileBytes, src, (uint32_t)C::kTileBytes, FULL(s));
+        if (++r == p.tpr) {
+          r = 0;
+          if (++j == p.n_b) { j = 0; ++b; }
+        }
       }
-      if (k_rot != nullptr) {
-        T* dst = k_rot + (row0 + t) * D;
+    }
+    return;
+  }
+  // ======================================= consumers: rotate, store, reduce =====================================
+  const int oct = tid % OCT, tok = tid / OCT;  // this thread's token of every tile, and its 8 pairs
+  const int i0 = oct * 8;
+  float2 tab[8];  // (cos, sin) of this thread's (token, pairs) for the current row
+  float acc[16];
+#pragma unroll
+  for (int u = 0; u < 16; ++u) acc[u] = 0.f;
+  bool fresh_row = true;
+  int pb = 0;  // `part` buffer of the next reduction event (double buffered: one barrier per event)
+  int mb = 1;  // `mid` buffer of the current row (flipped at every row change)
+
+  for (int k = 0; k < nt; ++k) {
+    const bool is_k = r < p.HK;
+    if (fresh_row) {
+      fresh_row = false;
+      mb ^= 1;
+      const long long pos_first = p.pos0 + (long long)j * kChunk;
+      const double pos = (double)(pos_first + tok);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) tab[u] = cos_sin_f32(pos, s_turns[i0 + u]);
+      if (p.HK > 0) {
+        // middle positions (reading R2: start + (S-1)/2), full fp64 sincos; read after a K tile's barrier
+        double2* mid = mid_base + mb * (kMaxGpc + 1) * half;
+        for (int idx = tid; idx < (p.gpc + 1) * half; idx += C::kConsumers) {
+          const int g = idx / half, i = idx - g * half;
+          const double pm = (g < p.gpc) ? (double)pos_first + (double)(g * p.gs) + 0.5 * (double)(p.gs - 1)
+                                        : (double)pos_first + 0.5 * (double)(kChunk - 1);
+          double sn, cs;
+          sincos(reduced_angle(pm, s_turns[i]), &sn, &cs);
+          mid[idx] = make_double2(cs, sn);
+        }
+      }
+    }
+    const int s = k % S;
+    mbar_wait(FULL(s), (uint32_t)(k / S) & 1u);
+    const T* rowp = reinterpret_cast<const T*>(smem + C::kTiles + s * C::kTileBytes) + tok * D;
+    float a[8], bb[8], ra[8], rb[8];
+    Io<T>::load8(rowp + i0, a);
+    Io<T>::load8(rowp + half + i0, bb);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(EMPTY(s));  // the values are in registers: the stage can be refilled
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const float2 c = tab[u];
+      ra[u] = fmaf(a[u], c.x, -(bb[u] * c.y));
+      rb[u] = fmaf(bb[u], c.x, a[u] * c.y);
+    }
+    {
+      T* dst = nullptr;
+      if (is_k) {
+        if (p.k_rot) dst = (T*)p.k_rot + (((size_t)b * p.HK + r) * p.N + (size_t)j * kChunk + tok) * D;
+      } else {
+        dst = (T*)p.q_rot + (((size_t)b * p.HQ + (r - p.HK)) * p.N + (size_t)j * kChunk + tok) * D;
+      }
+      if (dst) {
         Io<T>::store8(dst + i0, ra);
         Io<T>::store8(dst + half + i0, rb);
       }
-      float* pr = rot_s + t * D;
-      float* pw = raw_s + t * D;
-      *reinterpret_cast<float4*>(pr + i0) = make_float4(ra[0], ra[1], ra[2], ra[3]);
-      *reinterpret_cast<float4*>(pr + i0 + 4) = make_float4(ra[4], ra[5], ra[6], ra[7]);
-      *reinterpret_cast<float4*>(pr + half + i0) = make_float4(rb[0], rb[1], rb[2], rb[3]);
-      *reinterpret_cast<float4*>(pr + half + i0 + 4) = make_float4(rb[4], rb[5], rb[6], rb[7]);
-      *reinterpret_cast<float4*>(pw + i0) = make_float4(a[0], a[1], a[2], a[3]);
-      *reinterpret_cast<float4*>(pw + i0 + 4) = make_float4(a[4], a[5], a[6], a[7]);
-      *reinterpret_cast<float4*>(pw + half + i0) = make_float4(bb[0], bb[1], bb[2], bb[3]);
-      *reinterpret_cast<float4*>(pw + half + i0 + 4) = make_float4(bb[4], bb[5], bb[6], bb[7]);
     }
-    __syncthreads();
-    // phase B: per (group, pair) sums in fp64, fixed order
-    if (b_active) {
-      double ra = 0.0, rb = 0.0, wa = 0.0, wb = 0.0;
-      for (int t = bg * gs; t < (bg + 1) * gs; ++t) {
-        ra += (double)rot_s[t * D + bi];
-        rb += (double)rot_s[t * D + half + bi];
-        wa += (double)raw_s[t * D + bi];
-        wb += (double)raw_s[t * D + half + bi];
+    const bool pool = !is_k && p.pooled != nullptr;
+    if (pool) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        acc[u] += ra[u];
+        acc[8 + u] += rb[u];
       }
-      dsum[(bg * 4 + 0) * half + bi] = ra;
-      dsum[(bg * 4 + 1) * half + bi] = rb;
-      dsum[(bg * 4 + 2) * half + bi] = wa;
-      dsum[(bg * 4 + 3) * half + bi] = wb;
-      if (group_sum != nullptr) {
-        double sa, sb;
-        const double inv = 1.0 / (double)gs;
-        if (bi < n_hi_g) {  // high-frequency pair: rotate per token, then average
-          sa = ra * inv;
-          sb = rb * inv;
-        } else {            // low-frequency pair: average raw keys, rotate at the middle position
-          double2 m = mid_g[bg * half + bi];
-          double ma = wa * inv, mb = wb * inv;
-          sa = ma * m.x - mb * m.y;
-          sb = mb * m.x + ma * m.y;
+    }
+    const bool unit_end = pool && ((r - p.HK + 1) % p.PG == 0);
+    float* part = part_base + (size_t)pb * NW * 2 * D;
+    if (is_k) {
+      // sums over the kTpw tokens of this warp (all inside one 16-token group), fixed order
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+#pragma unroll
+        for (int off = OCT; off < 32; off <<= 1) {
+          ra[u] += __shfl_xor_sync(0xffffffffu, ra[u], off);
+          rb[u] += __shfl_xor_sync(0xffffffffu, rb[u], off);
+          a[u] += __shfl_xor_sync(0xffffffffu, a[u], off);
+          bb[u] += __shfl_xor_sync(0xffffffffu, bb[u], off);
         }
-        float* dst = group_sum + (((size_t)b * Hkv + h) * (size_t)(n_b * gpc) + (size_t)j * gpc + bg) * D;
-        dst[bi] = (float)sa;
-        dst[half + bi] = (float)sb;
+      }
+      if (lane < OCT) {
+        float* pr = part + (size_t)warp * 2 * D;  // [rot D][raw D]
+        *reinterpret_cast<float4*>(pr + i0) = make_float4(ra[0], ra[1], ra[2], ra[3]);
+        *reinterpret_cast<float4*>(pr + i0 + 4) = make_float4(ra[4], ra[5], ra[6], ra[7]);
+        *reinterpret_cast<float4*>(pr + half + i0) = make_float4(rb[0], rb[1], rb[2], rb[3]);
+        *reinterpret_cast<float4*>(pr + half + i0 + 4) = make_float4(rb[4], rb[5], rb[6], rb[7]);
+        *reinterpret_cast<float4*>(pr + D + i0) = make_float4(a[0], a[1], a[2], a[3]);
+        *reinterpret_cast<float4*>(pr + D + i0 + 4) = make_float4(a[4], a[5], a[6], a[7]);
+        *reinterpret_cast<float4*>(pr + D + half + i0) = make_float4(bb[0], bb[1], bb[2], bb[3]);
+        *reinterpret_cast<float4*>(pr + D + half + i0 + 4) = make_float4(bb[4], bb[5], bb[6], bb[7]);
+      }
+    } else if (unit_end) {
+      // pooled query of the unit: reduce over the tokens of the warp, then (after the barrier) over the warps
+#pragma unroll
+      for (int u = 0; u < 16; ++u) {
+#pragma unroll
+        for (int off = OCT; off < 32; off <<= 1) acc[u] += __shfl_xor_sync(0xffffffffu, acc[u], off);
+      }
+      if (lane < OCT) {
+        float* pr = part + (size_t)warp * D;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          pr[i0 + u] = acc[u];
+          pr[half + i0 + u] = acc[8 + u];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 16; ++u) acc[u] = 0.f;
+    }
+    if (is_k) {
+      consumer_sync(C::kConsumers);
+      pb ^= 1;
+      const double2* mid = mid_base + mb * (kMaxGpc + 1) * half;
+      for (int idx = tid; idx < (p.gpc + 1) * half; idx += C::kConsumers) {
+        const int g = idx / half, i = idx - g * half;
+        const bool chunk_level = g == p.gpc;
+        const int span = chunk_level ? kChunk : p.gs;
+        const int w0 = chunk_level ? 0 : g * p.gs / C::kTpw;
+        const int w1 = chunk_level ? NW : (g + 1) * p.gs / C::kTpw;
+        double sra = 0.0, srb = 0.0, swa = 0.0, swb = 0.0;
+        for (int w = w0; w < w1; ++w) {  // warp w holds tokens [w*kTpw, (w+1)*kTpw)
+          const float* pr = part + (size_t)w * 2 * D;
+          sra += (double)pr[i];
+          srb += (double)pr[half + i];
+          swa += (double)pr[D + i];
+          swb += (double)pr[D + half + i];
+        }
+        const double inv = 1.0 / (double)span;
+        const int n_hi = chunk_level ? p.n_hi_c : p.n_hi_g;
+        double sa, sb;
+        if (i < n_hi) {  // high-frequency pair: rotate per token, then average
+          sa = sra * inv;
+          sb = srb * inv;
+        } else {         // low-frequency pair: average raw keys, rotate at the middle position
+          const double2 m = mid[idx];
+          const double ma = swa * inv, mbv = swb * inv;
+          sa = ma * m.x - mbv * m.y;
+          sb = mbv * m.x + ma * m.y;
+        }
+        float* dstp = nullptr;
+        if (chunk_level) {
+          if (p.chunk_sum) dstp = p.chunk_sum + (((size_t)b * p.HK + r) * p.n_b + j) * D;
+        } else if (p.group_sum) {
+          dstp = p.group_sum + (((size_t)b * p.HK + r) * (size_t)(p.n_b * p.gpc) + (size_t)j * p.gpc + g) * D;
+        }
+        if (dstp) {
+          dstp[i] = (float)sa;
+          dstp[half + i] = (float)sb;
+        }
+      }
+    } else if (unit_end) {
+      consumer_sync(C::kConsumers);
+      pb ^= 1;
+      if (tid < D) {
+        double sum = 0.0;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) sum += (double)part[w * D + tid];
+        const int n_pg = p.HQ / p.PG, pg = (r - p.HK) / p.PG;
+        p.pooled[(((size_t)b * n_pg + pg) * p.n_b + j) * D + tid] = (float)(sum / (double)(p.PG * kChunk));
       }
     }
-    __syncthreads();
-    if (chunk_sum != nullptr && threadIdx.x < half) {
-      const int i = threadIdx.x;
-      double ra = 0.0, rb = 0.0, wa = 0.0, wb = 0.0;
-      for (int g = 0; g < gpc; ++g) {
-        ra += dsum[(g * 4 + 0) * half + i];
-        rb += dsum[(g * 4 + 1) * half + i];
-        wa += dsum[(g * 4 + 2) * half + i];
-        wb += dsum[(g * 4 + 3) * half + i];
-      }
-      const double inv = 1.0 / (double)kChunk;
-      double sa, sb;
-      if (i < n_hi_c) {
-        sa = ra * inv;
-        sb = rb * inv;
-      } else {
-        double2 m = mid_c[i];
-        double ma = wa * inv, mb = wb * inv;
-        sa = ma * m.x - mb * m.y;
-        sb = mb * m.x + ma * m.y;
-      }
-      float* dst = chunk_sum + (((size_t)b * Hkv + h) * n_b + j) * D;
-      dst[i] = (float)sa;
-      dst[half + i] = (float)sb;
+    if (++r == p.tpr) {
+      r = 0;
+      fresh_row = true;
+      if (++j == p.n_b) { j = 0; ++b; }
     }
-    // The next head's phase A only writes rot_s/raw_s (phase B readers are past the barrier above); its phase B
-    // writes dsum only after the next __syncthreads(), which the finalising threads also reach.
   }
 }
 
-// Largest divisor hpc of n_items (a multiple of `quantum`) that still leaves >= target CTAs.
-int pick_per_cta(int n_items, int quantum, long long other_ctas, long long target) {
-  int best = quantum;
-  for (int hpc = quantum; hpc <= n_items; hpc += quantum) {
-    if (n_items % hpc) continue;
-    if (other_ctas * (n_items / hpc) >= target) best = hpc;
+template <typename T, int D>
+hga_status launch_stream_t(const RopeFreq& f, RsParams p, long long rows, cudaStream_t s) {
+  using C = RsCfg<T, D>;
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    HGA_CUDA_OK(cudaGetDevice(&dev));
+    HGA_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
   }
-  return best;
-}
-
-template <typename T, int D>
-hga_status launch_rope_t(const Derived& d, const RopeFreq& f, const void* x_raw, int n_heads, void* x_rot, float* pooled,
-                         cudaStream_t s) {
-  const int pool_heads = pooled ? n_heads / d.Hkv : 1;
-  const int hpc = pick_per_cta(n_heads, pool_heads, (long long)d.n_b * d.B, 1024);
-  const size_t smem = sizeof(float2) * kChunk * (D / 2) + sizeof(double) * (kThreads / (D / 16)) * D;
-  auto kern = rope_pool_kernel<T, D>;
-  HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid(d.n_b, n_heads / hpc, d.B);
-  kern<<<grid, kThreads, smem, s>>>(f, (const T*)x_raw, (T*)x_rot, pooled, n_heads, d.N, d.n_b, hpc, pool_heads, d.pos0);
+  p.tpr = p.HK + p.HQ;
+  p.total_tiles = rows * p.tpr;
+  const long long units = rows * (p.HK + (p.HQ ? p.HQ / p.PG : 0));
+  const int ctas_per_sm = C::kCtasPerSm;
+  const long long cap = (long long)n_sm * ctas_per_sm;
+  const int grid = (int)(units < cap ? units : cap);
+  if (grid <= 0) return HGA_OK;
+  auto kern = rope_stream_kernel<T, D>;
+  HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kBytes));
+  kern<<<grid, C::kThreads, C::kBytes, s>>>(f, p);
   return launch_status();
 }
 
-template <typename T, int D>
-hga_status launch_summaries_t(const Derived& d, const RopeFreq& f, const void* k_raw, void* k_rot, float* chunk_sum,
-                              float* group_sum, cudaStream_t s) {
-  const int hpc = pick_per_cta(d.Hkv, 1, (long long)d.n_b * d.B, 1024);
-  constexpr int half = D / 2;
-  const size_t smem = sizeof(float2) * kChunk * half + 2 * sizeof(float) * kChunk * D +
-                      sizeof(double2) * ((kChunk / 16) + 1) * half + sizeof(double) * (kChunk / 16) * 4 * half;
-  auto kern = summaries_kernel<T, D>;
-  HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid(d.n_b, d.Hkv / hpc, d.B);
-  kern<<<grid, kThreads, smem, s>>>(f, (const T*)k_raw, (T*)k_rot, chunk_sum, group_sum, d.Hkv, d.N, d.n_b, hpc, d.gs,
-                                    d.n_hi_c, d.n_hi_g, d.pos0);
-  return launch_status();
+hga_status launch_stream(const Derived& d, const RopeFreq& f, const RsParams& p, cudaStream_t s) {
+  const long long rows = (long long)d.B * d.n_b;
+  if (d.bf16_io) {
+    return d.D == 128 ? launch_stream_t<__nv_bfloat16, 128>(f, p, rows, s) : launch_stream_t<__nv_bfloat16, 64>(f, p, rows, s);
+  }
+  return d.D == 128 ? launch_stream_t<float, 128>(f, p, rows, s) : launch_stream_t<float, 64>(f, p, rows, s);
+}
+
+RsParams base_params(const Derived& d) {
+  RsParams p = {};
+  p.N = d.N; p.n_b = d.n_b;
+  p.PG = 1;
+  p.gs = d.gs; p.gpc = d.gpc; p.n_hi_c = d.n_hi_c; p.n_hi_g = d.n_hi_g;
+  p.pos0 = d.pos0;
+  return p;
 }
 
 }  // namespace
 
+// S0 + S1 in one launch (hga_prefill): K tiles and Q tiles of a row share the position tables.
+hga_status launch_rope_summaries(const Derived& d, const RopeFreq& f, const void* q_raw, void* q_rot, float* pooled,
+                                 const void* k_raw, void* k_rot, float* chunk_sum, float* group_sum, cudaStream_t s) {
+  RsParams p = base_params(d);
+  p.q_raw = q_raw; p.q_rot = q_rot; p.pooled = pooled;
+  p.HQ = d.Hq; p.PG = pooled ? d.G : 1;
+  p.k_raw = k_raw; p.k_rot = k_rot; p.chunk_sum = chunk_sum; p.group_sum = group_sum;
+  p.HK = d.Hkv;
+  return launch_stream(d, f, p, s);
+}
+
 hga_status launch_rope(const Derived& d, const RopeFreq& f, const void* x_raw, int n_heads, void* x_rot, float* pooled,
                        cudaStream_t s) {
-  if (d.bf16_io) {
-    return d.D == 128 ? launch_rope_t<__nv_bfloat16, 128>(d, f, x_raw, n_heads, x_rot, pooled, s)
-                      : launch_rope_t<__nv_bfloat16, 64>(d, f, x_raw, n_heads, x_rot, pooled, s);
-  }
-  return d.D == 128 ? launch_rope_t<float, 128>(d, f, x_raw, n_heads, x_rot, pooled, s)
-                    : launch_rope_t<float, 64>(d, f, x_raw, n_heads, x_rot, pooled, s);
+  RsParams p = base_params(d);
+  p.q_raw = x_raw; p.q_rot = x_rot; p.pooled = pooled;
+  p.HQ = n_heads; p.PG = pooled ? n_heads / d.Hkv : 1;
+  return launch_stream(d, f, p, s);
 }
 
 hga_status launch_summaries(const Derived& d, const RopeFreq& f, const void* k_raw, void* k_rot, float* chunk_sum,
                             float* group_sum, cudaStream_t s) {
-  if (d.bf16_io) {
-    return d.D == 128 ? launch_summaries_t<__nv_bfloat16, 128>(d, f, k_raw, k_rot, chunk_sum, group_sum, s)
-                      : launch_summaries_t<__nv_bfloat16, 64>(d, f, k_raw, k_rot, chunk_sum, group_sum, s);
-  }
-  return d.D == 128 ? launch_summaries_t<float, 128>(d, f, k_raw, k_rot, chunk_sum, group_sum, s)
-                    : launch_summaries_t<float, 64>(d, f, k_raw, k_rot, chunk_sum, group_sum, s);
+  RsParams p = base_params(d);
+  p.k_raw = k_raw; p.k_rot = k_rot; p.chunk_sum = chunk_sum; p.group_sum = group_sum;
+  p.HK = d.Hkv;
+  return launch_stream(d, f, p, s);
 }
 
 }  // namespace hga
