@@ -3,7 +3,8 @@
 //   score_kernel : scores[b,kv,j,c] = <q_pooled[b,kv,j], chunk_sum[b,kv,c]> for the lower triangle c < j, as a tiled
 //                  contraction with fp64 accumulation (inputs are fp32, converted once when staged in shared memory).
 //                  Scores decide integer index sets that must match an fp64 oracle, so no TF32/bf16 tensor cores here.
-//   select_kernel: one warp per (b, kv, block j): top-K_c of the middle candidates by repeated warp arg-max
+//   select_fast_kernel (K_c <= 32) / select_generic_kernel: one warp per (b, kv, block j): top-K_c of the middle
+//                  candidates by repeated warp arg-max
 //                  (shuffle reduction on (score desc, index asc)), ascending compaction by ballot scan; then the
 //                  C/g_s groups of every kept chunk are scored (warp-cooperative fp64 dot products) and the top-K_g kept.
 #include <math_constants.h>
@@ -15,10 +16,14 @@ namespace hga {
 namespace {
 
 constexpr int kTile = 64;
-constexpr int kSlab = 16;
+constexpr int kSlab = 32;
 
-__global__ void __launch_bounds__(256) score_kernel(const float* __restrict__ q_pooled, const float* __restrict__ chunk_sum,
-                                                    float* __restrict__ scores, int n_b, int D, int F, int L_eff) {
+// 64 x 64 score tile per 64-thread CTA, 8 x 8 accumulators per thread: per k-step a thread reads 8 + 8 doubles for
+// 64 DFMAs, which balances the shared-memory pipe against the fp64 pipe (a 4 x 4 micro-tile is LDS-bound 2:1).
+// Thread (tx, ty) owns rows 16a + 2ty + {0,1} and columns 16b + 2tx + {0,1} (a, b = 0..3): every LDS.128 of a
+// quarter-warp covers 128 contiguous bytes (S) or one broadcast address (Q).
+__global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_pooled, const float* __restrict__ chunk_sum,
+                                                   float* __restrict__ scores, int n_b, int D, int F, int L_eff) {
   // triangular tile index -> (tj, tc), tc <= tj
   const int ti = blockIdx.x;
   int tj = (int)((sqrtf(8.0f * (float)ti + 1.0f) - 1.0f) * 0.5f);
@@ -36,51 +41,61 @@ __global__ void __launch_bounds__(256) score_kernel(const float* __restrict__ q_
   const float* S = chunk_sum + slice * (size_t)n_b * D;
   float* out = scores + slice * (size_t)n_b * n_b;
 
-  __shared__ __align__(16) double Qs[kSlab][kTile + 2];
-  __shared__ __align__(16) double Ss[kSlab][kTile + 2];
-  const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
-  const int lr = threadIdx.x / 4, lp = threadIdx.x % 4;  // loader: row, float4 part of the 16-wide slab
-  double acc[4][4];
+  __shared__ __align__(16) double Qs[kSlab][kTile];
+  __shared__ __align__(16) double Ss[kSlab][kTile];
+  const int tid = threadIdx.x, tx = tid % 8, ty = tid / 8;
+  double acc[8][8];
 #pragma unroll
-  for (int a = 0; a < 4; ++a)
+  for (int a = 0; a < 8; ++a)
 #pragma unroll
-    for (int b = 0; b < 4; ++b) acc[a][b] = 0.0;
+    for (int b = 0; b < 8; ++b) acc[a][b] = 0.0;
 
   for (int k0 = 0; k0 < D; k0 += kSlab) {
-    float4 qv = make_float4(0.f, 0.f, 0.f, 0.f), sv = qv;
-    if (j0 + lr < n_b) qv = *reinterpret_cast<const float4*>(Q + (size_t)(j0 + lr) * D + k0 + lp * 4);
-    if (c0 + lr < n_b) sv = *reinterpret_cast<const float4*>(S + (size_t)(c0 + lr) * D + k0 + lp * 4);
     __syncthreads();  // previous slab fully consumed
-    Qs[lp * 4 + 0][lr] = (double)qv.x; Qs[lp * 4 + 1][lr] = (double)qv.y;
-    Qs[lp * 4 + 2][lr] = (double)qv.z; Qs[lp * 4 + 3][lr] = (double)qv.w;
-    Ss[lp * 4 + 0][lr] = (double)sv.x; Ss[lp * 4 + 1][lr] = (double)sv.y;
-    Ss[lp * 4 + 2][lr] = (double)sv.z; Ss[lp * 4 + 3][lr] = (double)sv.w;
+    {
+      // thread `tid` stages row tid of both operands: 32 consecutive floats each, converted once to double
+      const bool qok = j0 + tid < n_b, sok = c0 + tid < n_b;
+      const float4* qp = reinterpret_cast<const float4*>(Q + (size_t)(j0 + tid) * D + k0);
+      const float4* sp = reinterpret_cast<const float4*>(S + (size_t)(c0 + tid) * D + k0);
+#pragma unroll
+      for (int v4 = 0; v4 < kSlab / 4; ++v4) {
+        const float4 qv = qok ? qp[v4] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 sv = sok ? sp[v4] : make_float4(0.f, 0.f, 0.f, 0.f);
+        Qs[v4 * 4 + 0][tid] = (double)qv.x; Qs[v4 * 4 + 1][tid] = (double)qv.y;
+        Qs[v4 * 4 + 2][tid] = (double)qv.z; Qs[v4 * 4 + 3][tid] = (double)qv.w;
+        Ss[v4 * 4 + 0][tid] = (double)sv.x; Ss[v4 * 4 + 1][tid] = (double)sv.y;
+        Ss[v4 * 4 + 2][tid] = (double)sv.z; Ss[v4 * 4 + 3][tid] = (double)sv.w;
+      }
+    }
     __syncthreads();
-#pragma unroll
+#pragma unroll 4
     for (int k = 0; k < kSlab; ++k) {
-      double2 q01 = *reinterpret_cast<const double2*>(&Qs[k][ty * 4]);
-      double2 q23 = *reinterpret_cast<const double2*>(&Qs[k][ty * 4 + 2]);
-      double2 s01 = *reinterpret_cast<const double2*>(&Ss[k][tx * 4]);
-      double2 s23 = *reinterpret_cast<const double2*>(&Ss[k][tx * 4 + 2]);
-      const double qa[4] = {q01.x, q01.y, q23.x, q23.y};
-      const double sb[4] = {s01.x, s01.y, s23.x, s23.y};
+      double qa[8], sb[8];
 #pragma unroll
-      for (int a = 0; a < 4; ++a)
+      for (int i = 0; i < 4; ++i) {
+        const double2 qv = *reinterpret_cast<const double2*>(&Qs[k][16 * i + 2 * ty]);
+        const double2 sv = *reinterpret_cast<const double2*>(&Ss[k][16 * i + 2 * tx]);
+        qa[2 * i] = qv.x; qa[2 * i + 1] = qv.y;
+        sb[2 * i] = sv.x; sb[2 * i + 1] = sv.y;
+      }
 #pragma unroll
-        for (int b = 0; b < 4; ++b) acc[a][b] = fma(qa[a], sb[b], acc[a][b]);  // d ascending: fixed order
+      for (int a = 0; a < 8; ++a)
+#pragma unroll
+        for (int b = 0; b < 8; ++b) acc[a][b] = fma(qa[a], sb[b], acc[a][b]);  // d ascending: fixed order
     }
   }
 #pragma unroll
-  for (int a = 0; a < 4; ++a) {
-    const int j = j0 + ty * 4 + a;
-    const int c = c0 + tx * 4;
-    if (j < n_b && c < n_b)  // n_b % 4 may be nonzero only for tiny problems; guard element-wise then
-    {
-      if (c + 3 < n_b && (n_b % 4) == 0) {
-        *reinterpret_cast<float4*>(out + (size_t)j * n_b + c) =
-            make_float4((float)acc[a][0], (float)acc[a][1], (float)acc[a][2], (float)acc[a][3]);
+  for (int a = 0; a < 8; ++a) {
+    const int j = j0 + 16 * (a / 2) + 2 * ty + (a % 2);
+    if (j >= n_b) continue;
+#pragma unroll
+    for (int b2 = 0; b2 < 4; ++b2) {
+      const int c = c0 + 16 * b2 + 2 * tx;
+      if (c + 1 < n_b && (n_b % 2) == 0) {
+        *reinterpret_cast<float2*>(out + (size_t)j * n_b + c) = make_float2((float)acc[a][2 * b2], (float)acc[a][2 * b2 + 1]);
       } else {
-        for (int b = 0; b < 4 && c + b < n_b; ++b) out[(size_t)j * n_b + c + b] = (float)acc[a][b];
+        if (c < n_b) out[(size_t)j * n_b + c] = (float)acc[a][2 * b2];
+        if (c + 1 < n_b) out[(size_t)j * n_b + c + 1] = (float)acc[a][2 * b2 + 1];
       }
     }
   }
@@ -107,7 +122,7 @@ __device__ __forceinline__ void warp_topk_mark(float* work, int n, int take, int
 }
 
 template <int D>
-__global__ void __launch_bounds__(128) select_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
+__global__ void __launch_bounds__(128) select_generic_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
                                                      const float* __restrict__ group_sum, int32_t* __restrict__ chunk_idx,
                                                      float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
                                                      int32_t* __restrict__ group_idx, float* __restrict__ group_score,
@@ -202,6 +217,200 @@ __global__ void __launch_bounds__(128) select_kernel(const float* __restrict__ s
   if (n_groups && lane == 0) n_groups[unit] = gcnt;
 }
 
+// ----------------------------------------------------------------------------------------------------------------
+// Fast selection path (K_c <= 32, at most 128 group candidates): one warp per (b, kv, block j).
+//   * the candidate row lives in shared memory with CONTIGUOUS ownership: lane l owns candidates [l*m, (l+1)*m)
+//     (m a power of two, rows padded to m+4 floats so that the LDS.128 of a quarter-warp is conflict-free), and
+//     keeps its best (value, offset) in registers;
+//   * a round = one redux.sync max over order-preserving integer keys + a ballot (the lowest tied lane owns the
+//     lowest index, R8) + a rescan of the winner lane's m candidates only;
+//   * the <= 32 winners sit one per lane and are ranked ascending by index with 32 shuffles;
+//   * group refinement scores one candidate per lane (fp64 FMA, d ascending, q in shared memory as doubles), so
+//     there is no cross-lane reduction at all; its top-K_g uses the same redux rounds on <= 4 values per lane.
+// ----------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t order_key(float v) {
+  const uint32_t u = __float_as_uint(v + 0.0f);  // -0 -> +0, so equal floats have equal keys
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+// Best (value, offset) of the m candidates at `col`; ascending scan with strict '>' keeps the lowest offset.
+__device__ __forceinline__ void lane_rescan(const float* col, int m, float& bv, int& bo) {
+  bv = -CUDART_INF_F;
+  bo = 0;
+  for (int o = 0; o < m; o += 4) {
+    const float4 v = *reinterpret_cast<const float4*>(col + o);
+    if (v.x > bv) { bv = v.x; bo = o; }
+    if (v.y > bv) { bv = v.y; bo = o + 1; }
+    if (v.z > bv) { bv = v.z; bo = o + 2; }
+    if (v.w > bv) { bv = v.w; bo = o + 3; }
+  }
+}
+
+template <int D>
+__global__ void __launch_bounds__(128) select_fast_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
+                                                          const float* __restrict__ group_sum, int32_t* __restrict__ chunk_idx,
+                                                          float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
+                                                          int32_t* __restrict__ group_idx, float* __restrict__ group_score,
+                                                          int32_t* __restrict__ n_groups, int n_units, int n_b, int n_g, int gpc,
+                                                          int F, int L_eff, int Kc, int Kg, int lm, int per_warp_bytes) {
+  extern __shared__ __align__(16) unsigned char smem_sel[];
+  constexpr unsigned kFull = 0xffffffffu;
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const int unit = blockIdx.x * (blockDim.x / 32) + warp;
+  if (unit >= n_units) return;  // warp-uniform; no block-wide barrier below
+  const int m = 1 << lm, stride = m + 4;
+  unsigned char* base = smem_sel + (size_t)warp * per_warp_bytes;
+  double* qd = reinterpret_cast<double*>(base);                 // [D]
+  float* work = reinterpret_cast<float*>(base + D * 8);         // [32][m + 4]
+  int* sel = reinterpret_cast<int*>(work + 32 * stride);        // [32]
+
+  const int j = unit % n_b;
+  const size_t slice = unit / n_b;  // b * Hkv + kv
+  const float* row = scores + (size_t)unit * n_b;
+  const int lo = F, hi = j - L_eff;
+  const int n = hi > lo ? hi - lo : 0;
+  int32_t* cidx = chunk_idx + (size_t)unit * Kc;
+  float* csc = chunk_score ? chunk_score + (size_t)unit * Kc : nullptr;
+
+  // ---- stage the row (coalesced reads), pad with -inf -------------------------------------------------------
+  const int n_lanes = (n + m - 1) >> lm;  // lanes that own at least one candidate
+  for (int c = lane; c < n_lanes * m; c += 32) {
+    const float v = c < n ? row[lo + c] : -CUDART_INF_F;
+    work[(c >> lm) * stride + (c & (m - 1))] = v;
+  }
+  __syncwarp();
+  float* col = work + lane * stride;
+  float bv = -CUDART_INF_F;
+  int bo = 0;
+  if (lane < n_lanes) lane_rescan(col, m, bv, bo);
+
+  // ---- top-K_c: one winner per round, kept in lane r ---------------------------------------------------------
+  const int take = min(Kc, n);
+  int win = 0x7fffffff;  // candidate index (relative to lo) of the winner this lane keeps
+  float wsc = 0.f;
+  if (take == n) {
+    if (lane < n) {
+      win = lane;
+      wsc = work[(lane >> lm) * stride + (lane & (m - 1))];
+    }
+  } else {
+    for (int r = 0; r < take; ++r) {
+      const uint32_t key = order_key(bv);
+      const uint32_t kmax = __reduce_max_sync(kFull, key);
+      const int owner = __ffs(__ballot_sync(kFull, key == kmax)) - 1;
+      const int cstar = __shfl_sync(kFull, lane * m + bo, owner);
+      const float vstar = __shfl_sync(kFull, bv, owner);
+      if (lane == r) {
+        win = cstar;
+        wsc = vstar;
+      }
+      if (lane == owner) {
+        col[bo] = -CUDART_INF_F;
+        lane_rescan(col, m, bv, bo);
+      }
+    }
+  }
+  // ---- ascending order: rank of this lane's winner among the winners ------------------------------------------
+  int rank = 0;
+#pragma unroll
+  for (int t = 0; t < 32; ++t) rank += (__shfl_sync(kFull, win, t) < win) ? 1 : 0;
+  const int cnt = take;
+  if (lane < cnt) {
+    cidx[rank] = lo + win;
+    sel[rank] = lo + win;
+    if (csc) csc[rank] = wsc;
+  }
+  for (int s = cnt + lane; s < Kc; s += 32) {
+    cidx[s] = -1;
+    if (csc) csc[s] = 0.f;
+  }
+  if (n_chunks && lane == 0) n_chunks[unit] = cnt;
+  if (Kg <= 0) return;
+
+  // ---- group refinement: candidate `cand` = group cand % gpc of kept chunk cand / gpc (ascending group order) -----
+  const int n_gc = cnt * gpc;  // <= 128
+  {
+    const float* qp = q_pooled + (size_t)unit * D;
+    for (int d = lane; d < D; d += 32) qd[d] = (double)qp[d];
+  }
+  __syncwarp();
+  const float* gbase = group_sum + slice * (size_t)n_g * D;
+  float gsc[4];   // score of candidate lane + 32*i
+  int gid[4];     // its group index
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int cand = lane + 32 * i;
+    gsc[i] = -CUDART_INF_F;
+    gid[i] = -1;
+    if (cand < n_gc) {
+      const int g = sel[cand / gpc] * gpc + cand % gpc;
+      const float4* gp = reinterpret_cast<const float4*>(gbase + (size_t)g * D);
+      double s = 0.0;
+#pragma unroll 4
+      for (int d4 = 0; d4 < D / 4; ++d4) {
+        const float4 v = __ldg(gp + d4);
+        const double2 q01 = *reinterpret_cast<const double2*>(qd + 4 * d4);
+        const double2 q23 = *reinterpret_cast<const double2*>(qd + 4 * d4 + 2);
+        s = fma(q01.x, (double)v.x, s);
+        s = fma(q01.y, (double)v.y, s);
+        s = fma(q23.x, (double)v.z, s);
+        s = fma(q23.y, (double)v.w, s);
+      }
+      gsc[i] = (float)s;
+      gid[i] = g;
+    }
+  }
+  const int gtake = min(Kg, n_gc);
+  unsigned taken = 0;  // bit i: candidate lane + 32*i is kept
+  if (gtake == n_gc) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      if (lane + 32 * i < n_gc) taken |= 1u << i;
+  } else {
+    float wv[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) wv[i] = gsc[i];
+    for (int r = 0; r < gtake; ++r) {
+      // lane-local best: value descending, candidate index ascending (i ascending == index ascending)
+      float lv = wv[0];
+      int li = 0;
+#pragma unroll
+      for (int i = 1; i < 4; ++i)
+        if (wv[i] > lv) { lv = wv[i]; li = i; }
+      const uint32_t key = order_key(lv);
+      const uint32_t kmax = __reduce_max_sync(kFull, key);
+      const bool tied = key == kmax;
+      const uint32_t cmin = __reduce_min_sync(kFull, tied ? (uint32_t)(lane + 32 * li) : 0xffffffffu);
+      if (tied && (uint32_t)(lane + 32 * li) == cmin) {
+        taken |= 1u << li;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+          if (i == li) wv[i] = -CUDART_INF_F;
+      }
+    }
+  }
+  // ascending compaction (candidates are in ascending group order)
+  int gcnt = 0;
+  int32_t* gidx = group_idx + (size_t)unit * Kg;
+  float* gscore = group_score ? group_score + (size_t)unit * Kg : nullptr;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const bool on = (taken >> i) & 1u;
+    const unsigned mk = __ballot_sync(kFull, on);
+    if (on) {
+      const int pos = gcnt + __popc(mk & ((1u << lane) - 1u));
+      gidx[pos] = gid[i];
+      if (gscore) gscore[pos] = gsc[i];
+    }
+    gcnt += __popc(mk);
+  }
+  for (int s = gcnt + lane; s < Kg; s += 32) {
+    gidx[s] = -1;
+    if (gscore) gscore[s] = 0.f;
+  }
+  if (n_groups && lane == 0) n_groups[unit] = gcnt;
+}
+
 }  // namespace
 
 hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
@@ -209,17 +418,36 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
   const int nt = (d.n_b + kTile - 1) / kTile;
   dim3 grid(nt * (nt + 1) / 2, d.Hkv, d.B);
-  score_kernel<<<grid, 256, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff);
+  score_kernel<<<grid, 64, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff);
   if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
 
   const int n_units = d.B * d.Hkv * d.n_b;
   const int kc_cap = d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b;
+  if (d.Kc <= 32 && kc_cap * d.gpc <= 128) {
+    // fast path: register/redux rounds, one candidate per lane in the group stage
+    const int n_max = d.n_b - d.F - d.L_eff > 1 ? d.n_b - d.F - d.L_eff : 1;
+    int lm = 2;
+    while ((32 << lm) < n_max) ++lm;
+    const int per_warp_bytes = d.D * 8 + 32 * ((1 << lm) + 4) * 4 + 32 * 4;
+    int warps = 4;
+    while (warps > 1 && (size_t)warps * per_warp_bytes > 200 * 1024) warps >>= 1;
+    const size_t smem = (size_t)warps * per_warp_bytes;
+    if (smem <= 200 * 1024) {
+      auto kern = d.D == 128 ? select_fast_kernel<128> : select_fast_kernel<64>;
+      HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
+                                                                   n_chunks, group_idx, group_score, n_groups, n_units,
+                                                                   d.n_b, d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, lm,
+                                                                   per_warp_bytes);
+      return launch_status();
+    }
+  }
   const int per_warp = d.n_b + 2 * kc_cap * d.gpc + kc_cap;
   int warps = 4;
   while (warps > 1 && (size_t)warps * per_warp * sizeof(float) > 200 * 1024) warps >>= 1;
   const size_t smem = (size_t)warps * per_warp * sizeof(float);
   if (smem > 200 * 1024) return HGA_ERR_UNSUPPORTED;
-  auto kern = d.D == 128 ? select_kernel<128> : select_kernel<64>;
+  auto kern = d.D == 128 ? select_generic_kernel<128> : select_generic_kernel<64>;
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
                                                                n_chunks, group_idx, group_score, n_groups, n_units, d.n_b,

@@ -73,6 +73,8 @@ SMALL = [
     ("d128_g3", 1, 1536, 6, 2, 128, 1e6, 5, 7, 2, 3),
     ("d64_g2_nolocal", 1, 1024, 4, 2, 64, 1e4, 3, 5, 0, 0),
     ("d128_g2_pos0", 1, 1024, 4, 2, 128, 1e6, 4, 16, 1, 2),
+    ("d64_g1_kc40", 1, 4096, 2, 2, 64, 1e4, 40, 50, 1, 1),   # K_c > 32: the generic selection kernel
+    ("d64_g2_kg_lt", 1, 2048, 4, 2, 64, 1e4, 20, 33, 1, 1),  # 80 group candidates, non-trivial top-33
 ]
 
 
