@@ -17,9 +17,12 @@
 // TMEM map (512 columns): S_t at t*128 (P_t overlays its first 64 columns), O_t at 256 + t*D.
 //
 // Softmax arithmetic: fp32, base-2 (scores scaled by scale*log2 e), running max refreshed lazily (only when it grows
-// by more than 2^8, which leaves the result mathematically unchanged), packed FFMA2/FADD2, FMNMX3 row max, and a
-// share of the exponentials evaluated on the FMA pipe (Cody-Waite + degree-3 polynomial, rel. error 7.5e-5, far
-// below the bf16 rounding of P) because MUFU.EX2 (16/clk/SM) would otherwise pace the 128x128 tiles.
+// by more than 2^8, which leaves the result mathematically unchanged), packed FFMA2/FADD2, FMNMX3 row max.
+// A share of the exponentials CAN be evaluated on the FMA pipe (Cody-Waite + degree-3 polynomial, rel. error
+// 7.5e-5, far below the bf16 rounding of P; HGA_S4_EMU_COUNT of every HGA_S4_EMU_PERIOD pairs).  It is off by
+// default: the softmax step sits on the latency chain softmax -> P V -> Q K^T -> softmax of its tile, and ncu shows
+// that chain bound by the warpgroup's instruction count, not by MUFU.EX2 throughput (XU pipe 43 % busy), so the
+// ~6 extra instructions per emulated element cost more than the MUFU slot they free.
 #include <cuda.h>
 #include <math_constants.h>
 
@@ -43,8 +46,14 @@ constexpr float kRescaleThreshold = 8.0f;  // log2 units
 constexpr int kRegsSoftmax = 200, kRegsEpi = 64, kRegsCtl = 48;  // 2*128*200 + 128*64 + 128*48 = 65536
 
 // exp2 on the FMA pipe for pairs p with (p % kEmuPeriod) < kEmuCount
-constexpr int kEmuPeriod = 4;
-constexpr int kEmuCount = 1;
+#ifndef HGA_S4_EMU_PERIOD
+#define HGA_S4_EMU_PERIOD 4
+#endif
+#ifndef HGA_S4_EMU_COUNT
+#define HGA_S4_EMU_COUNT 0  // measured at c5 (S4 ms): 0/4 -> 0.987, 1/8 -> 1.033, 1/4 -> 1.063, 3/8 -> 1.097, 1/2 -> 1.144
+#endif
+constexpr int kEmuPeriod = HGA_S4_EMU_PERIOD;
+constexpr int kEmuCount = HGA_S4_EMU_COUNT;
 
 struct Tc2Params {
   int B, Hq, Hkv, N, n_b, G;
