@@ -190,6 +190,13 @@ typedef struct hga_buffers {
 HGA_API hga_status hga_prefill(const hga_params* p, const hga_buffers* buf, void* stream);
 
 /*
+ * Instrumented hga_prefill: the same three launches groups with CUDA events recorded on `stream` between them; the
+ * call synchronises `stream` and writes the elapsed milliseconds of {S0+S1 (one fused launch), S2+S3, S4} to the HOST
+ * array stage_ms[3].  For measurement only (bench.py's per-stage roofline inside the real call sequence).
+ */
+HGA_API hga_status hga_prefill_profile(const hga_params* p, const hga_buffers* buf, void* stream, float* stage_ms_host);
+
+/*
  * Host-buffer path.  A plan owns every device buffer of one prefill pass for `p` plus a private stream.
  * hga_host_prefill copies q/k/v from HOST memory (pinned for full speed; pageable works), runs S0..S4, copies `out`
  * (and, if non-null, group_idx [batch,n_kv_heads,seq/chunk,topk_groups] and lse) back to HOST memory and returns

@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     hga_build_summaries,
     hga_default_n_hi,
     hga_prefill,
+    hga_prefill_profile,
     hga_rope,
     hga_route,
     hga_validate,

@@ -65,6 +65,7 @@ def load_library():
     lib.hga_route.argtypes = [P, F, F, F, V, F, V, V, F, V, V, C.c_size_t, V]
     lib.hga_attend.argtypes = [P, V, V, V, V, V, F, V]
     lib.hga_prefill.argtypes = [P, C.POINTER(_CBuffers), V]
+    lib.hga_prefill_profile.argtypes = [P, C.POINTER(_CBuffers), V, C.POINTER(C.c_float)]
     lib.hga_host_plan_create.argtypes = [P, C.POINTER(C.c_void_p)]
     lib.hga_host_prefill.argtypes = [V, V, V, V, V, V, V]
     lib.hga_host_plan_destroy.argtypes = [V]
@@ -280,12 +281,7 @@ class PrefillBuffers:
         )
 
 
-def hga_prefill(p: Params, q_raw: torch.Tensor, k_raw: torch.Tensor, v: torch.Tensor,
-                buf: Optional[PrefillBuffers] = None, want_lse: bool = True) -> PrefillBuffers:
-    """S0..S4 on the current stream (one C call)."""
-    assert q_raw.dtype == p.torch_io and k_raw.dtype == p.torch_io and v.dtype == p.torch_io
-    if buf is None:
-        buf = PrefillBuffers.allocate(p, q_raw.device)
+def _cbuffers(q_raw, k_raw, v, buf, want_lse):
     cb = _CBuffers()
     cb.q_raw, cb.k_raw, cb.v = q_raw.data_ptr(), k_raw.data_ptr(), v.data_ptr()
     for name in ("q_rot", "k_rot", "q_pooled", "chunk_sum", "group_sum", "chunk_idx", "chunk_score", "n_chunks",
@@ -293,8 +289,27 @@ def hga_prefill(p: Params, q_raw: torch.Tensor, k_raw: torch.Tensor, v: torch.Te
         setattr(cb, name, getattr(buf, name).data_ptr())
     cb.lse = buf.lse.data_ptr() if want_lse else None
     cb.workspace_bytes = buf.workspace.numel()
+    return cb
+
+
+def hga_prefill(p: Params, q_raw: torch.Tensor, k_raw: torch.Tensor, v: torch.Tensor,
+                buf: Optional[PrefillBuffers] = None, want_lse: bool = True) -> PrefillBuffers:
+    """S0..S4 on the current stream (one C call)."""
+    assert q_raw.dtype == p.torch_io and k_raw.dtype == p.torch_io and v.dtype == p.torch_io
+    if buf is None:
+        buf = PrefillBuffers.allocate(p, q_raw.device)
+    cb = _cbuffers(q_raw, k_raw, v, buf, want_lse)
     _check(load_library().hga_prefill(C.byref(p.c()), C.byref(cb), _stream()), "hga_prefill")
     return buf
+
+
+def hga_prefill_profile(p: Params, q_raw: torch.Tensor, k_raw: torch.Tensor, v: torch.Tensor, buf: PrefillBuffers,
+                        want_lse: bool = True):
+    """hga_prefill with events between its launches; synchronises and returns [S0+S1, S2+S3, S4] in ms."""
+    cb = _cbuffers(q_raw, k_raw, v, buf, want_lse)
+    ms = (C.c_float * 3)()
+    _check(load_library().hga_prefill_profile(C.byref(p.c()), C.byref(cb), _stream(), ms), "hga_prefill_profile")
+    return [float(x) for x in ms]
 
 
 class HostPlan:

@@ -165,7 +165,7 @@ hga_status hga_attend(const hga_params* p, const void* q_rot, const void* k_rot,
   return launch_attend_simt(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
 }
 
-hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) {
+static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* stream, cudaEvent_t* ev) {
   if (!b) return HGA_ERR_INVALID_ARG;
   Derived d;
   RopeFreq f;
@@ -175,14 +175,39 @@ hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) 
   if (!aligned16(b->q_raw) || !aligned16(b->q_rot) || !aligned16(b->q_pooled) || !aligned16(b->k_raw) ||
       !aligned16(b->k_rot) || !aligned16(b->chunk_sum) || !aligned16(b->group_sum))
     return HGA_ERR_INVALID_ARG;
+  cudaStream_t cs = (cudaStream_t)stream;
+  if (ev) HGA_CUDA_OK(cudaEventRecord(ev[0], cs));
   // S0 + S1 in one launch: the K tiles and Q tiles of a (batch, chunk) row share the position tables
-  st = launch_rope_summaries(d, f, b->q_raw, b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum,
-                             (cudaStream_t)stream);
+  st = launch_rope_summaries(d, f, b->q_raw, b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum, cs);
   if (st != HGA_OK) return st;
+  if (ev) HGA_CUDA_OK(cudaEventRecord(ev[1], cs));
   st = hga_route(p, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
                  b->group_score, b->n_groups, b->workspace, b->workspace_bytes, stream);
   if (st != HGA_OK) return st;
-  return hga_attend(p, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, stream);
+  if (ev) HGA_CUDA_OK(cudaEventRecord(ev[2], cs));
+  st = hga_attend(p, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, stream);
+  if (st != HGA_OK) return st;
+  if (ev) HGA_CUDA_OK(cudaEventRecord(ev[3], cs));
+  return HGA_OK;
+}
+
+hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) {
+  return prefill_impl(p, b, stream, nullptr);
+}
+
+hga_status hga_prefill_profile(const hga_params* p, const hga_buffers* b, void* stream, float* stage_ms_host) {
+  if (!stage_ms_host) return HGA_ERR_INVALID_ARG;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  hga_status st = HGA_OK;
+  for (int i = 0; i < 4 && st == HGA_OK; ++i)
+    if (cudaEventCreate(&ev[i]) != cudaSuccess) st = HGA_ERR_CUDA;
+  if (st == HGA_OK) st = prefill_impl(p, b, stream, ev);
+  if (st == HGA_OK && cudaEventSynchronize(ev[3]) != cudaSuccess) st = HGA_ERR_CUDA;
+  for (int i = 0; i < 3 && st == HGA_OK; ++i)
+    if (cudaEventElapsedTime(&stage_ms_host[i], ev[i], ev[i + 1]) != cudaSuccess) st = HGA_ERR_CUDA;
+  for (int i = 0; i < 4; ++i)
+    if (ev[i]) cudaEventDestroy(ev[i]);
+  return st;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -191,7 +216,12 @@ hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) 
 struct hga_host_plan {
   hga_params p;
   Derived d;
-  cudaStream_t stream;
+  cudaStream_t stream;       // compute
+  cudaStream_t s_in, s_out;  // host->device / device->host copies (PCIe is full duplex: they overlap)
+  cudaEvent_t *ev_in, *ev_done;  // [n_parts]
+  // the work is pipelined over parts: runs of kv_per_part KV heads of one batch item (batch_per_part == 1), or
+  // batch_per_part whole batch items (kv_per_part == n_kv_heads)
+  int n_parts, kv_per_part, batch_per_part;
   void* arena;
   size_t arena_bytes;
   hga_buffers buf;
@@ -238,6 +268,28 @@ hga_status hga_host_plan_create(const hga_params* p, hga_host_plan** out_plan) {
   if (cudaStreamCreateWithFlags(&pl->stream, cudaStreamNonBlocking) != cudaSuccess) {
     cudaFree(pl->arena); delete pl; return HGA_ERR_CUDA;
   }
+  // parts: units (batch, KV head) are independent in every stage and contiguous in every tensor, so the copy-in of
+  // part i+1 and the copy-out of part i-1 overlap the kernels of part i.  Fewest parts >= 4 (fewer, larger parts
+  // keep both the kernels and the PCIe transfers efficient).
+  pl->kv_per_part = d.Hkv;
+  pl->batch_per_part = 1;
+  if (d.B >= 4) {
+    for (int nb = d.B; nb >= 1; --nb)
+      if (d.B % nb == 0 && d.B / nb >= 4) { pl->batch_per_part = nb; break; }
+  } else {
+    pl->kv_per_part = 1;
+    for (int m = d.Hkv; m >= 1; --m)
+      if (d.Hkv % m == 0 && d.B * (d.Hkv / m) >= 4) { pl->kv_per_part = m; break; }
+  }
+  pl->n_parts = (d.B / pl->batch_per_part) * (d.Hkv / pl->kv_per_part);
+  pl->ev_in = new (std::nothrow) cudaEvent_t[pl->n_parts]();
+  pl->ev_done = new (std::nothrow) cudaEvent_t[pl->n_parts]();
+  bool ok = pl->ev_in && pl->ev_done && cudaStreamCreateWithFlags(&pl->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&pl->s_out, cudaStreamNonBlocking) == cudaSuccess;
+  for (int i = 0; ok && i < pl->n_parts; ++i)
+    ok = cudaEventCreateWithFlags(&pl->ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&pl->ev_done[i], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) { cudaFree(pl->arena); delete[] pl->ev_in; delete[] pl->ev_done; delete pl; return HGA_ERR_CUDA; }
   char* base = (char*)pl->arena;
   size_t off = 0;
   auto take = [&](size_t s) { void* r = base + off; off += align_up(s); return r; };
@@ -256,24 +308,62 @@ hga_status hga_host_plan_create(const hga_params* p, hga_host_plan** out_plan) {
 hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k_host, const void* v_host,
                             void* out_host, int32_t* group_idx_host, float* lse_host) {
   if (!pl || !q_host || !k_host || !v_host || !out_host) return HGA_ERR_INVALID_ARG;
-  cudaStream_t s = pl->stream;
-  HGA_CUDA_OK(cudaMemcpyAsync((void*)pl->buf.q_raw, q_host, pl->q_bytes, cudaMemcpyHostToDevice, s));
-  HGA_CUDA_OK(cudaMemcpyAsync((void*)pl->buf.k_raw, k_host, pl->kv_bytes, cudaMemcpyHostToDevice, s));
-  HGA_CUDA_OK(cudaMemcpyAsync((void*)pl->buf.v, v_host, pl->kv_bytes, cudaMemcpyHostToDevice, s));
-  hga_buffers b = pl->buf;
-  if (!lse_host) b.lse = nullptr;
-  hga_status st = hga_prefill(&pl->p, &b, (void*)s);
-  if (st != HGA_OK) return st;
-  HGA_CUDA_OK(cudaMemcpyAsync(out_host, pl->buf.out, pl->out_bytes, cudaMemcpyDeviceToHost, s));
-  if (group_idx_host && pl->d.Kg > 0)
-    HGA_CUDA_OK(cudaMemcpyAsync(group_idx_host, pl->buf.group_idx, pl->gidx_bytes, cudaMemcpyDeviceToHost, s));
-  if (lse_host) HGA_CUDA_OK(cudaMemcpyAsync(lse_host, pl->buf.lse, pl->lse_bytes, cudaMemcpyDeviceToHost, s));
-  HGA_CUDA_OK(cudaStreamSynchronize(s));
+  const Derived& d = pl->d;
+  const int m = pl->kv_per_part, nb = pl->batch_per_part;
+  hga_params sp = pl->p;  // one part: nb batch items x m KV heads (m*G query heads)
+  sp.batch = nb;
+  sp.n_kv_heads = m;
+  sp.n_q_heads = m * d.G;
+  const size_t e = d.bf16_io ? 2 : 4, eo = d.bf16_out ? 2 : 4;
+  const size_t q_part = (size_t)nb * m * d.G * d.N * d.D, kv_part = (size_t)nb * m * d.N * d.D;
+  const size_t unit_part = (size_t)nb * m * d.n_b;
+  const size_t lse_part = (size_t)nb * m * d.G * d.N;
+  auto off = [](const void* base, size_t bytes) { return (void*)((const char*)base + bytes); };
+  for (int i = 0; i < pl->n_parts; ++i) {
+    // parts tile every tensor contiguously: element offsets are i * part size
+    const size_t qo = (size_t)i * q_part, ko = (size_t)i * kv_part, uo = (size_t)i * unit_part;
+    HGA_CUDA_OK(cudaMemcpyAsync(off(pl->buf.k_raw, ko * e), off(k_host, ko * e), kv_part * e, cudaMemcpyHostToDevice, pl->s_in));
+    HGA_CUDA_OK(cudaMemcpyAsync(off(pl->buf.q_raw, qo * e), off(q_host, qo * e), q_part * e, cudaMemcpyHostToDevice, pl->s_in));
+    HGA_CUDA_OK(cudaMemcpyAsync(off(pl->buf.v, ko * e), off(v_host, ko * e), kv_part * e, cudaMemcpyHostToDevice, pl->s_in));
+    HGA_CUDA_OK(cudaEventRecord(pl->ev_in[i], pl->s_in));
+    HGA_CUDA_OK(cudaStreamWaitEvent(pl->stream, pl->ev_in[i], 0));
+    hga_buffers b = pl->buf;
+    b.q_raw = off(pl->buf.q_raw, qo * e); b.q_rot = off(pl->buf.q_rot, qo * e);
+    b.k_raw = off(pl->buf.k_raw, ko * e); b.k_rot = off(pl->buf.k_rot, ko * e);
+    b.v = off(pl->buf.v, ko * e);
+    b.q_pooled = pl->buf.q_pooled + uo * d.D; b.chunk_sum = pl->buf.chunk_sum + uo * d.D;
+    b.group_sum = pl->buf.group_sum + uo * d.gpc * d.D;
+    b.chunk_idx = pl->buf.chunk_idx + uo * (d.Kc > 0 ? d.Kc : 1);
+    b.group_idx = pl->buf.group_idx + uo * (d.Kg > 0 ? d.Kg : 1);
+    b.out = off(pl->buf.out, qo * eo);
+    b.lse = lse_host ? pl->buf.lse + (size_t)i * lse_part : nullptr;
+    // the score workspace is shared: parts run one after another on the compute stream
+    hga_status st = hga_prefill(&sp, &b, (void*)pl->stream);
+    if (st != HGA_OK) return st;
+    HGA_CUDA_OK(cudaEventRecord(pl->ev_done[i], pl->stream));
+    HGA_CUDA_OK(cudaStreamWaitEvent(pl->s_out, pl->ev_done[i], 0));
+    HGA_CUDA_OK(cudaMemcpyAsync(off(out_host, qo * eo), b.out, q_part * eo, cudaMemcpyDeviceToHost, pl->s_out));
+    if (group_idx_host && d.Kg > 0)
+      HGA_CUDA_OK(cudaMemcpyAsync(group_idx_host + uo * d.Kg, b.group_idx, unit_part * d.Kg * 4, cudaMemcpyDeviceToHost,
+                                  pl->s_out));
+    if (lse_host)
+      HGA_CUDA_OK(cudaMemcpyAsync(lse_host + (size_t)i * lse_part, b.lse, lse_part * 4, cudaMemcpyDeviceToHost, pl->s_out));
+  }
+  HGA_CUDA_OK(cudaStreamSynchronize(pl->s_out));
+  HGA_CUDA_OK(cudaStreamSynchronize(pl->stream));
   return HGA_OK;
 }
 
 void hga_host_plan_destroy(hga_host_plan* pl) {
   if (!pl) return;
+  for (int i = 0; i < pl->n_parts; ++i) {
+    cudaEventDestroy(pl->ev_in[i]);
+    cudaEventDestroy(pl->ev_done[i]);
+  }
+  delete[] pl->ev_in;
+  delete[] pl->ev_done;
+  cudaStreamDestroy(pl->s_in);
+  cudaStreamDestroy(pl->s_out);
   cudaStreamDestroy(pl->stream);
   cudaFree(pl->arena);
   delete pl;
