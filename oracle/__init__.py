@@ -6,6 +6,7 @@ package.  It never imports paper_2606_30709_b200 and shares no code with it.
 from .hga_oracle import (  # noqa: F401
     OracleParams,
     SliceResult,
+    StepResult,
     attend_block,
     build,
     default_n_hi,
@@ -20,5 +21,6 @@ from .hga_oracle import (  # noqa: F401
     round_io,
     route_chunks,
     route_groups,
+    step,
     summaries,
 )

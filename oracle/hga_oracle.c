@@ -317,10 +317,12 @@ int hga_oracle_key_set(int j, int C, int gs, int F, int L, const int* group_idx,
 /*   k_rot [N,D], v [N,D]: rotated+rounded keys, values as given (fp64 copies)                         */
 /*   out [G,C,D], lse [G,C] (natural log of the softmax denominator, incl. the max), n_keys [C] optional */
 /* ------------------------------------------------------------------------------------------------ */
-int hga_oracle_attend_block(const double* q_blk, const double* k_rot, const double* v, int G, int N, int D,
-                            int C, int gs, int F, int L, int j, const int* group_idx, int n_group_slots,
-                            double scale, double* out, double* lse, int* n_keys) {
-  if ((j + 1) * C > N) return HGA_ORACLE_ERR_ARG;
+/* Rows [r0, r0+W) of block j: q_rows [G,W,D]; k_rot / v hold at least the tokens 0 .. j*C+r0+W-1.      */
+/* out [G,W,D], lse [G,W], n_keys [W] optional.  hga_oracle_attend_block is the case r0 = 0, W = C.     */
+int hga_oracle_attend_rows(const double* q_rows, const double* k_rot, const double* v, int G, int n_tok_avail,
+                           int D, int C, int gs, int F, int L, int j, int r0, int W, const int* group_idx,
+                           int n_group_slots, double scale, double* out, double* lse, int* n_keys) {
+  if (r0 < 0 || W < 0 || r0 + W > C || j * C + r0 + W > n_tok_avail) return HGA_ORACLE_ERR_ARG;
   if (scale <= 0.0) scale = 1.0 / sqrt((double)D);
   int n_tok = (j + 1) * C;
   unsigned char* vis = (unsigned char*)malloc((size_t)n_tok);
@@ -331,9 +333,9 @@ int hga_oracle_attend_block(const double* q_blk, const double* k_rot, const doub
   }
   double* logit = (double*)malloc(sizeof(double) * (size_t)n_tok);
   for (int h = 0; h < G; ++h)
-    for (int r = 0; r < C; ++r) {
-      const double* q = q_blk + ((size_t)h * C + r) * D;
-      int t = j * C + r; /* query token; keys u <= t only (causal, Eq. 1) */
+    for (int r = 0; r < W; ++r) {
+      const double* q = q_rows + ((size_t)h * W + r) * D;
+      int t = j * C + r0 + r; /* query token; keys u <= t only (causal, Eq. 1) */
       double m = -INFINITY;
       int cnt = 0;
       for (int u = 0; u <= t; ++u) {
@@ -343,7 +345,7 @@ int hga_oracle_attend_block(const double* q_blk, const double* k_rot, const doub
         ++cnt;
       }
       double den = 0.0;
-      double* o = out + ((size_t)h * C + r) * D;
+      double* o = out + ((size_t)h * W + r) * D;
       for (int d = 0; d < D; ++d) o[d] = 0.0;
       for (int u = 0; u <= t; ++u) {
         if (!vis[u]) continue;
@@ -352,12 +354,20 @@ int hga_oracle_attend_block(const double* q_blk, const double* k_rot, const doub
         for (int d = 0; d < D; ++d) o[d] += w * v[(size_t)u * D + d];
       }
       for (int d = 0; d < D; ++d) o[d] /= den;
-      if (lse) lse[(size_t)h * C + r] = m + log(den);
+      if (lse) lse[(size_t)h * W + r] = m + log(den);
       if (n_keys && h == 0) n_keys[r] = cnt;
     }
   free(logit);
   free(vis);
   return HGA_ORACLE_OK;
+}
+
+int hga_oracle_attend_block(const double* q_blk, const double* k_rot, const double* v, int G, int N, int D,
+                            int C, int gs, int F, int L, int j, const int* group_idx, int n_group_slots,
+                            double scale, double* out, double* lse, int* n_keys) {
+  if ((j + 1) * C > N) return HGA_ORACLE_ERR_ARG;
+  return hga_oracle_attend_rows(q_blk, k_rot, v, G, N, D, C, gs, F, L, j, 0, C, group_idx, n_group_slots, scale,
+                                out, lse, n_keys);
 }
 
 /* Dense causal attention, Eq. (1), for the rows of block j: every token u <= t is a key.  */
@@ -488,5 +498,78 @@ done:
   free(S_c);
   free(S_g);
   free(vd);
+  return rc;
+}
+
+/* ------------------------------------------------------------------------------------------------ */
+/* N1  One STREAMING STEP (chunk-by-chunk prefill, single-token decode, ragged prompt tail): the      */
+/*     store/router cycle of PAPER.md:158 -- "appending a newly closed chunk, reading chunk summaries  */
+/*     for routing, fetching group summaries for the second routing level, and gathering exact token   */
+/*     K/V" -- for the token window [t0, t1) of the active chunk j = t0 / C, t1 <= (j+1) C.             */
+/*     "Vectorized prefill and chunk-by-chunk decode must agree" (Table 7 :291-292).      */
+/*  The function is handed ONLY the history a step may see, so causality is structural:                */
+/*     q_win [G, W, D] raw queries of the window (W = t1 - t0);  k_raw, v [t1, D]: tokens 0 .. t1-1.    */
+/*  Reading R17: the routing query of a step is the mean of the rotated queries of the     */
+/*  rows processed in that step over the G heads (O3 restricted to the window): a whole block gives    */
+/*  exactly O3; a single decode token routes with its own GQA-pooled query.                            */
+/*  Order: O1 (keys 0..t1-1, window queries) -> O2 for the CLOSED chunks c < j only       */
+/*  -> O3 over the window -> O4, O5 with block index j -> O6 for the window's rows.                     */
+/*  Outputs (each may be NULL): q_pooled [D]; chunk_idx/score [Kc], n_chunks[1]; group_idx/score [Kg],  */
+/*  n_groups[1]; out [G,W,D]; lse [G,W].                                                               */
+/* ------------------------------------------------------------------------------------------------ */
+int hga_oracle_step(const hga_oracle_params* p, const float* q_win, const float* k_raw, const float* v,
+                    int64_t t0, int64_t t1, double* q_pooled, int* chunk_idx, double* chunk_score,
+                    int* n_chunks, int* group_idx, double* group_score, int* n_groups, double* out, double* lse) {
+  const int G = p->G, D = p->D, C = p->C, gs = p->gs;
+  if (G <= 0 || D <= 0 || (D & 1) || C <= 0 || gs <= 0 || C % gs || p->F < 0 || p->L < 0 || p->Kc < 0 || p->Kg < 0)
+    return HGA_ORACLE_ERR_ARG;
+  if (t0 < 0 || t1 <= t0) return HGA_ORACLE_ERR_ARG;
+  const int j = (int)(t0 / C), W = (int)(t1 - t0), r0 = (int)(t0 - (int64_t)j * C);
+  if (t1 > (int64_t)(j + 1) * C) return HGA_ORACLE_ERR_ARG; /* a step stays inside the active chunk */
+  const int n_hist = (int)t1, n_closed = j, gpc = C / gs;
+  for (size_t i = 0; i < (size_t)G * W * D; ++i)
+    if (!isfinite(q_win[i])) return HGA_ORACLE_ERR_NONFINITE;
+  for (size_t i = 0; i < (size_t)n_hist * D; ++i)
+    if (!isfinite(k_raw[i]) || !isfinite(v[i])) return HGA_ORACLE_ERR_NONFINITE;
+  int rc = HGA_ORACLE_OK;
+  double* k_rot = (double*)malloc(sizeof(double) * (size_t)n_hist * D);
+  double* vd = (double*)malloc(sizeof(double) * (size_t)n_hist * D);
+  double* S_c = (double*)malloc(sizeof(double) * (size_t)(n_closed > 0 ? n_closed : 1) * D);
+  double* S_g = (double*)malloc(sizeof(double) * (size_t)(n_closed > 0 ? n_closed * gpc : 1) * D);
+  double* q_rot = (double*)malloc(sizeof(double) * (size_t)G * W * D);
+  double* qbar = (double*)malloc(sizeof(double) * (size_t)D);
+  int* cidx = (int*)malloc(sizeof(int) * (size_t)(p->Kc > 0 ? p->Kc : 1));
+  int* gidx = (int*)malloc(sizeof(int) * (size_t)(p->Kg > 0 ? p->Kg : 1));
+  /* O1 keys of the visible history, O2 summaries of the closed chunks (from RAW keys, R7) */
+  rc |= hga_oracle_rope(k_raw, n_hist, D, p->pos0, p->base, k_rot);
+  if (n_closed > 0) {
+    rc |= hga_oracle_summaries(k_raw, n_closed * C, D, C, p->n_hi_chunk, p->pos0, p->base, S_c);
+    rc |= hga_oracle_summaries(k_raw, n_closed * C, D, gs, p->n_hi_group, p->pos0, p->base, S_g);
+  }
+  hga_oracle_round_io(k_rot, (size_t)n_hist * D, p->io_bf16);
+  for (size_t i = 0; i < (size_t)n_hist * D; ++i) vd[i] = (double)v[i];
+  /* O1 window queries, O3 over the window (R17) */
+  for (int h = 0; h < G; ++h)
+    rc |= hga_oracle_rope(q_win + (size_t)h * W * D, W, D, p->pos0 + t0, p->base, q_rot + (size_t)h * W * D);
+  rc |= hga_oracle_pool_queries(q_rot, G, W, D, W, qbar); /* a [G,W,D] tensor is one block of length W */
+  if (rc) goto done;
+  if (q_pooled) memcpy(q_pooled, qbar, sizeof(double) * (size_t)D);
+  {
+    /* O4, O5 over the closed chunks */
+    int nc = hga_oracle_route_chunks(qbar, S_c, n_closed, D, j, p->F, p->L, p->Kc, cidx, chunk_score, NULL);
+    int ng = hga_oracle_route_groups(qbar, S_g, D, gpc, cidx, nc, p->Kg, gidx, group_score, NULL);
+    if (chunk_idx) memcpy(chunk_idx, cidx, sizeof(int) * (size_t)p->Kc);
+    if (group_idx) memcpy(group_idx, gidx, sizeof(int) * (size_t)p->Kg);
+    if (n_chunks) *n_chunks = nc;
+    if (n_groups) *n_groups = ng;
+  }
+  /* O6 for the window's rows */
+  if (out) {
+    hga_oracle_round_io(q_rot, (size_t)G * W * D, p->io_bf16);
+    rc = hga_oracle_attend_rows(q_rot, k_rot, vd, G, n_hist, D, C, gs, p->F, p->L, j, r0, W, gidx, p->Kg, p->scale,
+                                out, lse, NULL);
+  }
+done:
+  free(k_rot); free(vd); free(S_c); free(S_g); free(q_rot); free(qbar); free(cidx); free(gidx);
   return rc;
 }

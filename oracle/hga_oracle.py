@@ -266,6 +266,40 @@ def prefill_slice(p: OracleParams, q_raw, k_raw, v, blocks=None, attend: bool = 
     return r
 
 
+@dataclasses.dataclass
+class StepResult:
+    q_pooled: np.ndarray  # [D]
+    chunk_idx: np.ndarray  # [Kc]
+    chunk_score: np.ndarray
+    n_chunks: int
+    group_idx: np.ndarray  # [Kg]
+    group_score: np.ndarray
+    n_groups: int
+    out: Optional[np.ndarray]  # [G,W,D]
+    lse: Optional[np.ndarray]  # [G,W]
+
+
+def step(p: OracleParams, q_win, k_hist, v_hist, t0: int, t1: int, attend: bool = True) -> StepResult:
+    """One streaming step (hga_oracle_step, N1): window [t0, t1) of the active chunk; q_win [G, t1-t0, D] raw queries
+    of the window, k_hist / v_hist [t1, D] -- ONLY tokens 0..t1-1 are handed over (p.N is ignored)."""
+    q_win, k_hist, v_hist = _f32(q_win), _f32(k_hist), _f32(v_hist)
+    G, W, D = q_win.shape
+    assert (G, D) == (p.G, p.D) and W == t1 - t0 and k_hist.shape == (t1, D) and v_hist.shape == (t1, D)
+    Kc, Kg = max(p.Kc, 1), max(p.Kg, 1)
+    qp = np.empty(D)
+    ci, cs, nc = np.empty(Kc, dtype=np.int32), np.empty(Kc), C.c_int(0)
+    gi, gsc, ng = np.empty(Kg, dtype=np.int32), np.empty(Kg), C.c_int(0)
+    out = np.empty((G, W, D)) if attend else None
+    lse = np.empty((G, W)) if attend else None
+    ps = p.c_struct()
+    rc = _L().hga_oracle_step(C.byref(ps), _p(q_win, C.c_float), _p(k_hist, C.c_float), _p(v_hist, C.c_float),
+                              C.c_int64(t0), C.c_int64(t1), _p(qp, C.c_double), _p(ci, C.c_int), _p(cs, C.c_double),
+                              C.byref(nc), _p(gi, C.c_int), _p(gsc, C.c_double), C.byref(ng), _p(out, C.c_double),
+                              _p(lse, C.c_double))
+    _check(rc, "step")
+    return StepResult(qp, ci[:p.Kc], cs[:p.Kc], nc.value, gi[:p.Kg], gsc[:p.Kg], ng.value, out, lse)
+
+
 def prefill(p: OracleParams, q_raw, k_raw, v, blocks=None, attend: bool = True, want_k_rot: bool = False):
     """Whole tensors: q_raw [B,Hq,N,D], k_raw/v [B,Hkv,N,D].  Returns {(b, kv_head): SliceResult}."""
     B, Hq = q_raw.shape[:2]

@@ -455,6 +455,75 @@ def test_config1_tiny_cpu_checkable():
     assert np.abs(r_all.out.transpose(1, 0, 2, 3).reshape(4, 1024, 64) - ref).max() < 1e-6
 
 
+# ----------------------------------------------------------------------------------------------------------------
+# N1 streaming step (chunk-by-chunk prefill, decode, ragged tail): Table 7 :291-292
+# ----------------------------------------------------------------------------------------------------------------
+def test_step_decode_full_coverage_equals_dense_recompute():
+    """Table 7 "HA decode vs full recompute": token-by-token steps with full coverage reproduce the dense causal row;
+    the step is handed only tokens 0..t, so the future cannot leak."""
+    tol = golden()["full_coverage_max_abs"]
+    w, q, k, v = small_problem(21, G=2, N=320, D=32)
+    pos = np.arange(320)
+    ref = sdpa_causal(rope_complex(q, pos[None].repeat(2, 0), w.rope_base), rope_complex(k, pos, w.rope_base), v)
+    p = oracle.OracleParams(G=2, N=320, D=32, F=1, L=1, Kc=5, Kg=20, base=w.rope_base)
+    for t in (0, 1, 63, 64, 65, 127, 200, 255, 256, 300, 319):
+        r = oracle.step(p, q[:, t:t + 1], k[:t + 1], v[:t + 1], t, t + 1)
+        assert r.out.shape == (2, 1, 32)
+        assert np.abs(r.out[:, 0] - ref[:, t]).max() < tol
+    # ragged prompt tail: window [256, 300) of the unfinished chunk 4, full coverage
+    r = oracle.step(p, q[:, 256:300], k[:300], v[:300], 256, 300)
+    assert np.abs(r.out - ref[:, 256:300]).max() < tol
+
+
+def test_step_sparse_window_against_direct_computation():
+    """A sparse step checked end to end against numpy/torch written here: pooled query = mean over the window's rows
+    and heads (R17), brute-force sort over the closed middle chunks and over the kept chunks' groups, softmax over
+    the explicitly enumerated key set.  Summaries come from oracle.summaries (pinned by P11-P15)."""
+    base, G, N, D, F, L, Kc, Kg = 1.0e4, 2, 640, 32, 1, 2, 3, 5
+    w, q, k, v = small_problem(22, G=G, N=N, D=D, clustered=True)
+    p = oracle.OracleParams(G=G, N=N, D=D, F=F, L=L, Kc=Kc, Kg=Kg, base=base, io_bf16=True)
+    kr_all = rope_complex(k, np.arange(N), base)
+    for (t0, t1) in ((576, 640), (600, 601), (639, 640), (448, 470), (130, 131), (64, 128)):
+        j = t0 // 64
+        r = oracle.step(p, q[:, t0:t1], k[:t1], v[:t1], t0, t1)
+        qr = rope_complex(q[:, t0:t1], np.arange(t0, t1)[None].repeat(G, 0), base)
+        qbar = qr.reshape(-1, D).mean(0)
+        assert np.abs(qbar - r.q_pooled).max() < 1e-13
+        S_c = oracle.summaries(k[: j * 64], 64, oracle.default_n_hi(D, base, 64), 0, base) if j else np.zeros((0, D))
+        S_g = oracle.summaries(k[: j * 64], 16, oracle.default_n_hi(D, base, 16), 0, base) if j else np.zeros((0, D))
+        cand = list(range(F, j - L))
+        order = sorted(cand, key=lambda c: (-float(S_c[c] @ qbar), c))[:Kc]
+        assert sorted(order) == [c for c in r.chunk_idx if c >= 0] and r.n_chunks == len(order)
+        gc = [4 * c + u for c in sorted(order) for u in range(4)]
+        gorder = sorted(sorted(gc, key=lambda g: (-float(S_g[g] @ qbar), g))[:Kg])
+        assert gorder == [g for g in r.group_idx if g >= 0] and r.n_groups == len(gorder)
+        # union set: sink chunks, local chunks, opened groups, current chunk up to the query
+        chunks = set(range(min(F, j))) | set(range(max(0, j - L), j))
+        base_keys = sorted({u for c in chunks for u in range(c * 64, c * 64 + 64)} |
+                           {u for g in gorder for u in range(g * 16, g * 16 + 16)})
+        kr, qrb = nearest_bf16(kr_all[:t1]), nearest_bf16(qr)
+        for h in range(G):
+            for row in sorted({0, (t1 - t0) // 2, t1 - t0 - 1}):
+                keys = np.array(base_keys + list(range(j * 64, t0 + row + 1)), dtype=np.int64)
+                pw = torch.softmax(torch.from_numpy(qrb[h, row] @ kr[keys].T / math.sqrt(D)), 0).numpy()
+                assert np.abs(pw @ v[keys].astype(np.float64) - r.out[h, row]).max() < 1e-12
+
+
+def test_step_chunk_by_chunk_equals_vectorised_prefill():
+    """PAPER.md:281: "vectorized prefill and chunk-by-chunk decode must agree up to floating-point noise" -- in the
+    oracle both run the same arithmetic in the same order, so whole-block steps agree exactly."""
+    w, q, k, v = small_problem(23, G=2, N=512, D=32, clustered=True)
+    p = oracle.OracleParams(G=2, N=512, D=32, Kc=2, Kg=5, base=w.rope_base, io_bf16=True)
+    full = oracle.prefill_slice(p, q, k, v)
+    for j in range(8):
+        r = oracle.step(p, q[:, j * 64:(j + 1) * 64], k[:(j + 1) * 64], v[:(j + 1) * 64], j * 64, (j + 1) * 64)
+        assert np.array_equal(r.chunk_idx, full.chunk_idx[j]) and np.array_equal(r.group_idx, full.group_idx[j])
+        assert np.array_equal(r.out, full.out[j]) and np.array_equal(r.lse, full.lse[j])
+        assert np.array_equal(r.q_pooled, full.q_pooled[j])
+    with pytest.raises(ValueError):
+        oracle.step(p, q[:, 60:70], k[:70], v[:70], 60, 70)  # a step never spans two chunks
+
+
 def test_c5_needle_group_is_routed_by_the_oracle():
     """BASELINE.json configs[4]: the planted 16-token needle group (cosine 0.9 with the final block's pooled rotated
     query) must appear in the routed set of the final block, at 10 / 50 / 90 % depth.  Stand-in for PAPER.md:214-231."""
