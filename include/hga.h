@@ -190,6 +190,33 @@ typedef struct hga_buffers {
 HGA_API hga_status hga_prefill(const hga_params* p, const hga_buffers* buf, void* stream);
 
 /*
+ * Streaming step: chunk-by-chunk prefill, single-token decode, ragged prompt tail.
+ * The store/router cycle of PAPER.md:158 ("appending a newly closed chunk, reading chunk summaries for routing,
+ * fetching group summaries for the second routing level, and gathering exact token K/V") for the token window
+ * [t_begin, t_end) of a cache whose capacity is p->seq tokens; "vectorized prefill and chunk-by-chunk decode must
+ * agree up to floating-point noise" (Table 7 :291-292).  hga_prefill is the window [0, p->seq).
+ *
+ * All tensors of `buf` keep the full-capacity layouts above and persist between calls (they ARE the cache).  On
+ * entry q_raw / k_raw / v hold the window's rows (k_raw also the earlier rows of a chunk that the window closes);
+ * K_rot, V and the summary tables hold what earlier calls left for tokens < t_begin.  The call
+ *   - rotates and stores Q_rot / K_rot rows of the window only (S0, S1);
+ *   - writes the chunk and group summaries of every chunk the window CLOSES, (c+1)*chunk <= t_end, from the raw keys of
+ *     the whole chunk -- an open chunk has no summary;
+ *   - routes every query block that intersects the window with q_pooled = mean of the rotated queries of the block's
+ *     rows INSIDE the window over the GQA group (reading R17: a whole block gives hga_prefill's pooled query, a single
+ *     decode token routes with its own pooled query) against the closed chunks before it (S2, S3); results go to row
+ *     j = t / chunk of q_pooled / chunk_idx / group_idx / ... (overwriting what an earlier step of the same block left);
+ *   - attends (S4): writes the out / lse rows of the window and no others.  Whole 64-row blocks go to the kernel
+ *     hga_attend would pick; a partial block (a window that starts or ends inside a chunk) goes to the fp32 SIMT kernel.
+ *     A window that starts inside a chunk must stay inside that chunk (one step of the active chunk).
+ * Values at positions >= t_end never influence a result and nothing there is written: the future part of the cache
+ * may be uninitialised (even NaN).  A chunk is summarised only by the call whose window closes it.
+ * Errors: HGA_ERR_INVALID_ARG for an empty/out-of-range window or one that starts inside a chunk and leaves it.
+ */
+HGA_API hga_status hga_prefill_window(const hga_params* p, const hga_buffers* buf, int64_t t_begin, int64_t t_end,
+                                      void* stream);
+
+/*
  * Instrumented hga_prefill: the same three launches groups with CUDA events recorded on `stream` between them; the
  * call synchronises `stream` and writes the elapsed milliseconds of {S0+S1 (one fused launch), S2+S3, S4} to the HOST
  * array stage_ms[3].  For measurement only (bench.py's per-stage roofline inside the real call sequence).

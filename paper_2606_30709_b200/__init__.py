@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     hga_default_n_hi,
     hga_prefill,
     hga_prefill_profile,
+    hga_prefill_window,
     hga_rope,
     hga_route,
     hga_validate,

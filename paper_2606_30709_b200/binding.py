@@ -65,6 +65,7 @@ def load_library():
     lib.hga_route.argtypes = [P, F, F, F, V, F, V, V, F, V, V, C.c_size_t, V]
     lib.hga_attend.argtypes = [P, V, V, V, V, V, F, V]
     lib.hga_prefill.argtypes = [P, C.POINTER(_CBuffers), V]
+    lib.hga_prefill_window.argtypes = [P, C.POINTER(_CBuffers), C.c_int64, C.c_int64, V]
     lib.hga_prefill_profile.argtypes = [P, C.POINTER(_CBuffers), V, C.POINTER(C.c_float)]
     lib.hga_host_plan_create.argtypes = [P, C.POINTER(C.c_void_p)]
     lib.hga_host_prefill.argtypes = [V, V, V, V, V, V, V]
@@ -300,6 +301,16 @@ def hga_prefill(p: Params, q_raw: torch.Tensor, k_raw: torch.Tensor, v: torch.Te
         buf = PrefillBuffers.allocate(p, q_raw.device)
     cb = _cbuffers(q_raw, k_raw, v, buf, want_lse)
     _check(load_library().hga_prefill(C.byref(p.c()), C.byref(cb), _stream()), "hga_prefill")
+    return buf
+
+
+def hga_prefill_window(p: Params, q_raw: torch.Tensor, k_raw: torch.Tensor, v: torch.Tensor, buf: PrefillBuffers,
+                       t_begin: int, t_end: int, want_lse: bool = True) -> PrefillBuffers:
+    """One streaming step over tokens [t_begin, t_end) of the cache held in (q_raw, k_raw, v, buf) (one C call)."""
+    assert q_raw.dtype == p.torch_io and k_raw.dtype == p.torch_io and v.dtype == p.torch_io
+    cb = _cbuffers(q_raw, k_raw, v, buf, want_lse)
+    _check(load_library().hga_prefill_window(C.byref(p.c()), C.byref(cb), t_begin, t_end, _stream()),
+           "hga_prefill_window")
     return buf
 
 

@@ -52,6 +52,7 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
   d->D = p->head_dim; d->half = p->head_dim / 2;
   d->C = p->chunk; d->gs = p->group; d->gpc = p->chunk / p->group;
   d->n_b = p->seq / p->chunk; d->n_g = p->seq / p->group;
+  d->jb = 0; d->nj = d->n_b; d->tw0 = 0; d->tw1 = p->seq;
   d->F = p->n_sink; d->L = p->n_local; d->L_eff = p->n_local > 1 ? p->n_local : 1;
   d->Kc = p->topk_chunks; d->Kg = p->topk_groups;
   d->n_hi_c = p->n_hi_chunk >= 0 ? p->n_hi_chunk : default_n_hi(p->head_dim, p->rope_base, p->chunk);
@@ -145,6 +146,41 @@ hga_status hga_route(const hga_params* p, const float* q_pooled, const float* ch
                       n_groups, (float*)workspace, (cudaStream_t)stream);
 }
 
+static hga_status attend_blocks(const Derived& d, int impl, const void* q_rot, const void* k_rot, const void* v,
+                                const int32_t* group_idx, void* out, float* lse, cudaStream_t cs) {
+  hga_status st;
+  if (impl == HGA_ATTEND_TCGEN05) {
+    st = launch_attend_tc2(d, q_rot, k_rot, v, group_idx, out, lse, cs);
+    if (st != HGA_ERR_UNSUPPORTED) return st;
+    impl = HGA_ATTEND_TCGEN05_ITEM;
+  }
+  if (impl == HGA_ATTEND_TCGEN05_ITEM) return launch_attend_tc(d, q_rot, k_rot, v, group_idx, out, lse, cs);
+  return launch_attend_simt(d, q_rot, k_rot, v, group_idx, out, lse, cs);
+}
+
+static hga_status attend_dispatch(const Derived& d, int impl, const void* q_rot, const void* k_rot, const void* v,
+                                  const int32_t* group_idx, void* out, float* lse, cudaStream_t cs) {
+  if (impl == HGA_ATTEND_AUTO) impl = d.bf16_io ? HGA_ATTEND_TCGEN05 : HGA_ATTEND_SIMT;
+  // The tcgen05 kernels work on whole 64-row blocks.  A partial block (decode step, partial append, ragged prompt
+  // tail) goes to the SIMT kernel, which masks rows and never reads a token at or past the end of the window.
+  const int last = d.jb + d.nj - 1;
+  const bool head_partial = d.tw0 % kChunk != 0, tail_partial = d.tw1 % kChunk != 0;
+  if (head_partial) return launch_attend_simt(d, q_rot, k_rot, v, group_idx, out, lse, cs);  // one block (validated)
+  if (!tail_partial) return attend_blocks(d, impl, q_rot, k_rot, v, group_idx, out, lse, cs);
+  if (d.nj > 1) {
+    Derived full = d;
+    full.nj = d.nj - 1;
+    full.tw1 = (long long)last * kChunk;
+    hga_status st = attend_blocks(full, impl, q_rot, k_rot, v, group_idx, out, lse, cs);
+    if (st != HGA_OK) return st;
+  }
+  Derived tail = d;
+  tail.jb = last;
+  tail.nj = 1;
+  tail.tw0 = (long long)last * kChunk;
+  return launch_attend_simt(tail, q_rot, k_rot, v, group_idx, out, lse, cs);
+}
+
 hga_status hga_attend(const hga_params* p, const void* q_rot, const void* k_rot, const void* v,
                       const int32_t* group_idx, void* out, float* lse, void* stream) {
   Derived d;
@@ -153,46 +189,54 @@ hga_status hga_attend(const hga_params* p, const void* q_rot, const void* k_rot,
   if (!q_rot || !k_rot || !v || !out) return HGA_ERR_INVALID_ARG;
   if (d.Kg > 0 && !group_idx) return HGA_ERR_INVALID_ARG;
   if (!aligned16(q_rot) || !aligned16(k_rot) || !aligned16(v) || !aligned16(out)) return HGA_ERR_INVALID_ARG;
-  int impl = p->attend_impl;
-  if (impl == HGA_ATTEND_AUTO) impl = d.bf16_io ? HGA_ATTEND_TCGEN05 : HGA_ATTEND_SIMT;
-  if (impl == HGA_ATTEND_TCGEN05) {
-    st = launch_attend_tc2(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
-    if (st != HGA_ERR_UNSUPPORTED) return st;
-    impl = HGA_ATTEND_TCGEN05_ITEM;
-  }
-  if (impl == HGA_ATTEND_TCGEN05_ITEM)
-    return launch_attend_tc(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
-  return launch_attend_simt(d, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
+  return attend_dispatch(d, p->attend_impl, q_rot, k_rot, v, group_idx, out, lse, (cudaStream_t)stream);
 }
 
-static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* stream, cudaEvent_t* ev) {
+static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* stream, cudaEvent_t* ev,
+                               long long t_begin, long long t_end) {
   if (!b) return HGA_ERR_INVALID_ARG;
   Derived d;
   RopeFreq f;
   hga_status st = derive(p, &d, &f);
   if (st != HGA_OK) return st;
-  if (!b->q_raw || !b->q_rot || !b->k_raw || !b->q_pooled || !b->k_rot || !b->chunk_sum) return HGA_ERR_INVALID_ARG;
-  if (!aligned16(b->q_raw) || !aligned16(b->q_rot) || !aligned16(b->q_pooled) || !aligned16(b->k_raw) ||
-      !aligned16(b->k_rot) || !aligned16(b->chunk_sum) || !aligned16(b->group_sum))
+  if (t_end < 0) t_end = d.N;
+  if (t_begin < 0 || t_begin >= t_end || t_end > d.N) return HGA_ERR_INVALID_ARG;
+  // a window that starts inside a chunk stays inside it (one step of the active chunk)
+  if (t_begin % kChunk != 0 && (t_begin / kChunk) != ((t_end - 1) / kChunk)) return HGA_ERR_INVALID_ARG;
+  d.tw0 = t_begin; d.tw1 = t_end;
+  d.jb = (int)(t_begin / kChunk);
+  d.nj = (int)((t_end + kChunk - 1) / kChunk) - d.jb;
+  if (!b->q_raw || !b->k_raw || !b->v || !b->q_rot || !b->k_rot || !b->q_pooled || !b->chunk_sum || !b->out ||
+      !b->chunk_idx)
     return HGA_ERR_INVALID_ARG;
+  if (d.Kg > 0 && (!b->group_sum || !b->group_idx)) return HGA_ERR_INVALID_ARG;
+  if (!aligned16(b->q_raw) || !aligned16(b->q_rot) || !aligned16(b->q_pooled) || !aligned16(b->k_raw) ||
+      !aligned16(b->k_rot) || !aligned16(b->chunk_sum) || !aligned16(b->group_sum) || !aligned16(b->v) ||
+      !aligned16(b->out))
+    return HGA_ERR_INVALID_ARG;
+  if (!b->workspace || !aligned16(b->workspace) || b->workspace_bytes < score_ws_bytes(d)) return HGA_ERR_WORKSPACE;
   cudaStream_t cs = (cudaStream_t)stream;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[0], cs));
   // S0 + S1 in one launch: the K tiles and Q tiles of a (batch, chunk) row share the position tables
   st = launch_rope_summaries(d, f, b->q_raw, b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum, cs);
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[1], cs));
-  st = hga_route(p, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
-                 b->group_score, b->n_groups, b->workspace, b->workspace_bytes, stream);
+  st = launch_route(d, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
+                    b->group_score, b->n_groups, (float*)b->workspace, cs);
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[2], cs));
-  st = hga_attend(p, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, stream);
+  st = attend_dispatch(d, p->attend_impl, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, cs);
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[3], cs));
   return HGA_OK;
 }
 
 hga_status hga_prefill(const hga_params* p, const hga_buffers* b, void* stream) {
-  return prefill_impl(p, b, stream, nullptr);
+  return prefill_impl(p, b, stream, nullptr, 0, -1);
+}
+
+hga_status hga_prefill_window(const hga_params* p, const hga_buffers* b, int64_t t_begin, int64_t t_end, void* stream) {
+  return prefill_impl(p, b, stream, nullptr, t_begin, t_end);
 }
 
 hga_status hga_prefill_profile(const hga_params* p, const hga_buffers* b, void* stream, float* stage_ms_host) {
@@ -201,7 +245,7 @@ hga_status hga_prefill_profile(const hga_params* p, const hga_buffers* b, void* 
   hga_status st = HGA_OK;
   for (int i = 0; i < 4 && st == HGA_OK; ++i)
     if (cudaEventCreate(&ev[i]) != cudaSuccess) st = HGA_ERR_CUDA;
-  if (st == HGA_OK) st = prefill_impl(p, b, stream, ev);
+  if (st == HGA_OK) st = prefill_impl(p, b, stream, ev, 0, -1);
   if (st == HGA_OK && cudaEventSynchronize(ev[3]) != cudaSuccess) st = HGA_ERR_CUDA;
   for (int i = 0; i < 3 && st == HGA_OK; ++i)
     if (cudaEventElapsedTime(&stage_ms_host[i], ev[i], ev[i + 1]) != cudaSuccess) st = HGA_ERR_CUDA;

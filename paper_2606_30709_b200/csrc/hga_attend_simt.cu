@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
                                                          const T* __restrict__ v, const int32_t* __restrict__ group_idx,
                                                          TO* __restrict__ out, float* __restrict__ lse, int Hq, int Hkv, int N,
                                                          int n_b, int F, int L_eff, int gs, int Kg, float scale,
-                                                         int list_cap) {
+                                                         int list_cap, int jb, int tw0, int tw1) {
   constexpr int KP = D + 4;  // padded row (keeps 16-byte alignment)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float* Qs = reinterpret_cast<float*>(smem_raw);  // [64][KP]
@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
   int* list = reinterpret_cast<int*>(a_s + 64);    // [list_cap] 16-token pieces
   __shared__ int s_count;
 
-  const int j = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
+  const int j = jb + blockIdx.x, h = blockIdx.y, b = blockIdx.z;
   const int G = Hq / Hkv, kv = h / G;
   const int32_t* gi = group_idx ? group_idx + (((size_t)b * Hkv + kv) * n_b + j) * Kg : nullptr;
   const int n_pieces = build_key_list(list, &s_count, j, F, L_eff, gs, Kg, gi);
@@ -72,8 +72,10 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
       float kvv = 0.f, vv = 0.f;
       if (r < np * 16) {
         size_t tok = (size_t)list[p0 + r / 16] * 16 + (r % 16);
-        kvv = ld_as_float(kbase + tok * D + c);
-        vv = ld_as_float(vbase + tok * D + c);
+        if (tok < (size_t)tw1) {  // rows past the token window are not part of the cache yet (zero, never NaN)
+          kvv = ld_as_float(kbase + tok * D + c);
+          vv = ld_as_float(vbase + tok * D + c);
+        }
       }
       Ks[r * KP + c] = kvv;
       Vs[r * D + c] = vv;
@@ -171,6 +173,8 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
 #pragma unroll
   for (int a = 0; a < 4; ++a) {
     const int row = ty * 4 + a;
+    const int t_abs = j * 64 + row;
+    if (t_abs < tw0 || t_abs >= tw1) continue;  // only the rows of the token window are written
     const float inv = 1.f / l_s[row];
 #pragma unroll
     for (int c = 0; c < OC; ++c) {
@@ -179,7 +183,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
       else obase[(size_t)row * D + tx + 16 * c] = __float2bfloat16_rn(val);
     }
   }
-  if (lse != nullptr && threadIdx.x < 64)
+  if (lse != nullptr && threadIdx.x < 64 && j * 64 + (int)threadIdx.x >= tw0 && j * 64 + (int)threadIdx.x < tw1)
     lse[((size_t)b * Hq + h) * N + (size_t)j * 64 + threadIdx.x] = m_s[threadIdx.x] + logf(l_s[threadIdx.x]);
 }
 
@@ -191,9 +195,9 @@ hga_status launch_t(const Derived& d, const void* q, const void* k, const void* 
   if (smem > 220 * 1024) return HGA_ERR_UNSUPPORTED;
   auto kern = attend_simt_kernel<T, TO, D>;
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid(d.n_b, d.Hq, d.B);
+  dim3 grid(d.nj, d.Hq, d.B);
   kern<<<grid, kT, smem, s>>>((const T*)q, (const T*)k, (const T*)v, gi, (TO*)out, lse, d.Hq, d.Hkv, d.N, d.n_b, d.F,
-                              d.L_eff, d.gs, d.Kg, d.scale, list_cap);
+                              d.L_eff, d.gs, d.Kg, d.scale, list_cap, d.jb, (int)d.tw0, (int)d.tw1);
   return launch_status();
 }
 

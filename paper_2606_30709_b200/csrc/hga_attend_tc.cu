@@ -34,6 +34,7 @@ using namespace tc;
 
 struct TcParams {
   int Hq, Hkv, N, n_b, G;
+  int jb;            // first query block of this launch (hga_prefill_window)
   int F, L_eff, gs, Kg;
   int n_mt;          // 128-row query tiles per unit = ceil(G/2)
   int ctas_per_unit; // ceil(n_mt/2)
@@ -80,7 +81,7 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
   int* list = reinterpret_cast<int*>(smem + L::kList);
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-  const int j = blockIdx.x / prm.ctas_per_unit;
+  const int j = prm.jb + blockIdx.x / prm.ctas_per_unit;
   const int cu = blockIdx.x % prm.ctas_per_unit;
   const int kv = blockIdx.y, b = blockIdx.z;
   const int mt0 = cu * 2;                               // first query tile of this CTA
@@ -340,6 +341,7 @@ hga_status launch_tc_t(const Derived& d, const void* q, const void* k, const voi
   using L = Smem<D>;
   TcParams prm;
   prm.Hq = d.Hq; prm.Hkv = d.Hkv; prm.N = d.N; prm.n_b = d.n_b; prm.G = d.G;
+  prm.jb = d.jb;
   prm.F = d.F; prm.L_eff = d.L_eff; prm.gs = d.gs; prm.Kg = d.Kg;
   prm.n_mt = (d.G + 1) / 2;
   prm.ctas_per_unit = (prm.n_mt + 1) / 2;
@@ -355,7 +357,7 @@ hga_status launch_tc_t(const Derived& d, const void* q, const void* k, const voi
     return HGA_ERR_CUDA;
   auto kern = attend_tc_kernel<D>;
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid(d.n_b * prm.ctas_per_unit, d.Hkv, d.B);
+  dim3 grid(d.nj * prm.ctas_per_unit, d.Hkv, d.B);
   kern<<<grid, kTcThreads, smem, s>>>(tmQ, tmK, tmV, gi, out, lse, prm);
   return launch_status();
 }

@@ -57,6 +57,7 @@ constexpr int kEmuCount = HGA_S4_EMU_COUNT;
 
 struct Tc2Params {
   int B, Hq, Hkv, N, n_b, G;
+  int jb, nj;  // query blocks [jb, jb + nj) of every (batch, kv head) are processed
   int F, L_eff, gs, Kg;
   int n_mt;           // 128-row query tiles per unit = ceil(G/2)
   int ctas_per_unit;  // ceil(n_mt/2)
@@ -94,11 +95,11 @@ __device__ __forceinline__ Item decode_item(int it, const Tc2Params& prm) {
   // (batch, kv head) outermost: the K/V of one head (c5: 33.5 MB) then stays L2-resident while Q streams through,
   // and the CTAs working at any moment share sink / routed / local lines.  Inside a head: j descending (longest
   // lists first, the short early blocks fill the tail), the CTAs of one unit adjacent.
-  const int per_head = prm.n_b * prm.ctas_per_unit;
+  const int per_head = prm.nj * prm.ctas_per_unit;
   Item r;
   const int bk = it / per_head;
   const int rem = it % per_head;
-  r.j = prm.n_b - 1 - rem / prm.ctas_per_unit;
+  r.j = prm.jb + prm.nj - 1 - rem / prm.ctas_per_unit;
   const int cu = rem % prm.ctas_per_unit;
   r.kv = bk % prm.Hkv;
   r.b = bk / prm.Hkv;
@@ -610,13 +611,14 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
   using L = Smem2<D>;
   Tc2Params prm;
   prm.B = d.B; prm.Hq = d.Hq; prm.Hkv = d.Hkv; prm.N = d.N; prm.n_b = d.n_b; prm.G = d.G;
+  prm.jb = d.jb; prm.nj = d.nj;
   prm.F = d.F; prm.L_eff = d.L_eff; prm.gs = d.gs; prm.Kg = d.Kg;
   prm.n_mt = (d.G + 1) / 2;
   prm.ctas_per_unit = (prm.n_mt + 1) / 2;
   prm.list_cap = max_key_pieces(d.F, d.L_eff, d.gs, d.Kg);
   prm.scale_log2 = d.scale * 1.4426950408889634f;
   prm.out_bf16 = d.bf16_out ? 1 : 0;
-  const long long n_items = (long long)d.B * d.Hkv * d.n_b * prm.ctas_per_unit;
+  const long long n_items = (long long)d.B * d.Hkv * d.nj * prm.ctas_per_unit;
   const size_t smem = (size_t)L::kList + 2 * sizeof(int) * (size_t)prm.list_cap;
   if (smem > 227 * 1024 || n_items >= (1ll << 31)) return HGA_ERR_UNSUPPORTED;
   if ((uint64_t)d.B * d.Hq * d.N >= (1ull << 31)) return HGA_ERR_UNSUPPORTED;

@@ -22,6 +22,8 @@ struct Derived {
   int B, N, Hq, Hkv, G, D, half;
   int C, gs, gpc;           // chunk, group, groups per chunk
   int n_b, n_g;             // chunks (= query blocks), groups per sequence
+  int jb, nj;               // blocks processed by this call: [jb, jb + nj); whole sequence: 0, n_b
+  long long tw0, tw1;       // token window of this call (hga_prefill_window); whole sequence: 0, N
   int F, L, L_eff, Kc, Kg;
   int n_hi_c, n_hi_g;
   long long pos0;

@@ -59,6 +59,8 @@ struct RsParams {
   float* chunk_sum;  // nullable
   float* group_sum;  // nullable
   int N, n_b;
+  int jb, nj;     // query blocks / chunks [jb, jb + nj) are processed (hga_prefill_window)
+  int tw0, tw1;   // token window: only rows t in [tw0, tw1) are stored and pooled; a chunk is summarised iff closed by tw1
   int HQ, PG;  // heads of the "Q" tensor (0: none), heads pooled together (a Q unit)
   int HK;      // heads of the "K" tensor (0: none)
   int gs, gpc, n_hi_c, n_hi_g;
@@ -135,7 +137,7 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
   // position of the CTA's first tile; every role advances (b, j, r) incrementally
   long long row0 = t0 / p.tpr;
   int r = (int)(t0 % p.tpr);
-  int b = (int)(row0 / p.n_b), j = (int)(row0 % p.n_b);
+  int b = (int)(row0 / p.nj), j = p.jb + (int)(row0 % p.nj);
 
   if (warp == NW) {
     // ===================================== producer: bulk loads into the ring ===================================
@@ -150,7 +152,7 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
         bulk_load(sbase + C::kTiles + s * C::kTileBytes, src, (uint32_t)C::kTileBytes, FULL(s));
         if (++r == p.tpr) {
           r = 0;
-          if (++j == p.n_b) { j = 0; ++b; }
+          if (++j == p.jb + p.nj) { j = p.jb; ++b; }
         }
       }
     }
@@ -203,6 +205,8 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
       ra[u] = fmaf(a[u], c.x, -(bb[u] * c.y));
       rb[u] = fmaf(bb[u], c.x, a[u] * c.y);
     }
+    const int t_abs = j * kChunk + tok;
+    const bool in_window = t_abs >= p.tw0 && t_abs < p.tw1;
     {
       T* dst = nullptr;
       if (is_k) {
@@ -210,13 +214,13 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
       } else {
         dst = (T*)p.q_rot + (((size_t)b * p.HQ + (r - p.HK)) * p.N + (size_t)j * kChunk + tok) * D;
       }
-      if (dst) {
+      if (dst && in_window) {
         Io<T>::store8(dst + i0, ra);
         Io<T>::store8(dst + half + i0, rb);
       }
     }
     const bool pool = !is_k && p.pooled != nullptr;
-    if (pool) {
+    if (pool && in_window) {
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
         acc[u] += ra[u];
@@ -297,7 +301,9 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
           sb = mbv * m.x + ma * m.y;
         }
         float* dstp = nullptr;
-        if (chunk_level) {
+        if ((j + 1) * kChunk > p.tw1) {
+          // the chunk is still open: only closed chunks are summarised
+        } else if (chunk_level) {
           if (p.chunk_sum) dstp = p.chunk_sum + (((size_t)b * p.HK + r) * p.n_b + j) * D;
         } else if (p.group_sum) {
           dstp = p.group_sum + (((size_t)b * p.HK + r) * (size_t)(p.n_b * p.gpc) + (size_t)j * p.gpc + g) * D;
@@ -315,13 +321,14 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
 #pragma unroll
         for (int w = 0; w < NW; ++w) sum += (double)part[w * D + tid];
         const int n_pg = p.HQ / p.PG, pg = (r - p.HK) / p.PG;
-        p.pooled[(((size_t)b * n_pg + pg) * p.n_b + j) * D + tid] = (float)(sum / (double)(p.PG * kChunk));
+        const int n_rows = min(p.tw1, (j + 1) * kChunk) - max(p.tw0, j * kChunk);  // rows of block j in the window
+        p.pooled[(((size_t)b * n_pg + pg) * p.n_b + j) * D + tid] = (float)(sum / (double)(p.PG * n_rows));
       }
     }
     if (++r == p.tpr) {
       r = 0;
       fresh_row = true;
-      if (++j == p.n_b) { j = 0; ++b; }
+      if (++j == p.jb + p.nj) { j = p.jb; ++b; }
     }
   }
 }
@@ -349,7 +356,7 @@ hga_status launch_stream_t(const RopeFreq& f, RsParams p, long long rows, cudaSt
 }
 
 hga_status launch_stream(const Derived& d, const RopeFreq& f, const RsParams& p, cudaStream_t s) {
-  const long long rows = (long long)d.B * d.n_b;
+  const long long rows = (long long)d.B * d.nj;
   if (d.bf16_io) {
     return d.D == 128 ? launch_stream_t<__nv_bfloat16, 128>(f, p, rows, s) : launch_stream_t<__nv_bfloat16, 64>(f, p, rows, s);
   }
@@ -359,6 +366,7 @@ hga_status launch_stream(const Derived& d, const RopeFreq& f, const RsParams& p,
 RsParams base_params(const Derived& d) {
   RsParams p = {};
   p.N = d.N; p.n_b = d.n_b;
+  p.jb = d.jb; p.nj = d.nj; p.tw0 = (int)d.tw0; p.tw1 = (int)d.tw1;
   p.PG = 1;
   p.gs = d.gs; p.gpc = d.gpc; p.n_hi_c = d.n_hi_c; p.n_hi_g = d.n_hi_g;
   p.pos0 = d.pos0;

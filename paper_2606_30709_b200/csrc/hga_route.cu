@@ -23,7 +23,7 @@ constexpr int kSlab = 32;
 // Thread (tx, ty) owns rows 16a + 2ty + {0,1} and columns 16b + 2tx + {0,1} (a, b = 0..3): every LDS.128 of a
 // quarter-warp covers 128 contiguous bytes (S) or one broadcast address (Q).
 __global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_pooled, const float* __restrict__ chunk_sum,
-                                                   float* __restrict__ scores, int n_b, int D, int F, int L_eff) {
+                                                   float* __restrict__ scores, int n_b, int D, int F, int L_eff, int jb, int je) {
   // triangular tile index -> (tj, tc), tc <= tj
   const int ti = blockIdx.x;
   int tj = (int)((sqrtf(8.0f * (float)ti + 1.0f) - 1.0f) * 0.5f);
@@ -33,7 +33,8 @@ __global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_p
   const int j0 = tj * kTile, c0 = tc * kTile;
   // any candidate (F <= c < j - L_eff) in this tile?  (block-uniform early exit)
   {
-    const int jmax = min(j0 + kTile - 1, n_b - 1), cmin = max(c0, F);
+    const int jmax = min(j0 + kTile - 1, je - 1), cmin = max(c0, F);
+    if (jmax < jb || j0 >= je) return;  // no row of [jb, je) in this tile (hga_prefill_window)
     if (cmin > jmax - L_eff - 1 || cmin > c0 + kTile - 1) return;
   }
   const size_t slice = (size_t)blockIdx.z * gridDim.y + blockIdx.y;  // b * Hkv + kv
@@ -87,7 +88,7 @@ __global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_p
 #pragma unroll
   for (int a = 0; a < 8; ++a) {
     const int j = j0 + 16 * (a / 2) + 2 * ty + (a % 2);
-    if (j >= n_b) continue;
+    if (j >= je || j < jb) continue;
 #pragma unroll
     for (int b2 = 0; b2 < 4; ++b2) {
       const int c = c0 + 16 * b2 + 2 * tx;
@@ -126,19 +127,20 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
                                                      const float* __restrict__ group_sum, int32_t* __restrict__ chunk_idx,
                                                      float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
                                                      int32_t* __restrict__ group_idx, float* __restrict__ group_score,
-                                                     int32_t* __restrict__ n_groups, int n_units, int n_b, int n_g, int gpc,
+                                                     int32_t* __restrict__ n_groups, int n_units, int jb, int nj, int n_b, int n_g, int gpc,
                                                      int F, int L_eff, int Kc, int Kg, int kc_cap, int per_warp_floats) {
   extern __shared__ __align__(16) float smem_f[];
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-  const int unit = blockIdx.x * (blockDim.x / 32) + warp;
-  if (unit >= n_units) return;  // warp-uniform; no block-wide barrier below
+  const int widx = blockIdx.x * (blockDim.x / 32) + warp;
+  if (widx >= n_units) return;  // warp-uniform; no block-wide barrier below
   float* work = smem_f + (size_t)warp * per_warp_floats;  // [n_b]
   float* gwork = work + n_b;                              // [kc_cap * gpc]
   float* gval = gwork + kc_cap * gpc;                     // [kc_cap * gpc]
   int* sel = reinterpret_cast<int*>(gval + kc_cap * gpc); // [kc_cap]
 
-  const int j = unit % n_b;
-  const size_t slice = unit / n_b;  // b * Hkv + kv
+  const int j = jb + widx % nj;          // blocks [jb, jb + nj) of every slice
+  const size_t slice = widx / nj;        // b * Hkv + kv
+  const size_t unit = slice * n_b + j;   // row of every [B, Hkv, n_b, ...] table
   const float* row = scores + (size_t)unit * n_b;
   const int lo = F, hi = j - L_eff;
   const int n = hi > lo ? hi - lo : 0;
@@ -251,21 +253,22 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
                                                           const float* __restrict__ group_sum, int32_t* __restrict__ chunk_idx,
                                                           float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
                                                           int32_t* __restrict__ group_idx, float* __restrict__ group_score,
-                                                          int32_t* __restrict__ n_groups, int n_units, int n_b, int n_g, int gpc,
+                                                          int32_t* __restrict__ n_groups, int n_units, int jb, int nj, int n_b, int n_g, int gpc,
                                                           int F, int L_eff, int Kc, int Kg, int lm, int per_warp_bytes) {
   extern __shared__ __align__(16) unsigned char smem_sel[];
   constexpr unsigned kFull = 0xffffffffu;
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-  const int unit = blockIdx.x * (blockDim.x / 32) + warp;
-  if (unit >= n_units) return;  // warp-uniform; no block-wide barrier below
+  const int widx = blockIdx.x * (blockDim.x / 32) + warp;
+  if (widx >= n_units) return;  // warp-uniform; no block-wide barrier below
   const int m = 1 << lm, stride = m + 4;
   unsigned char* base = smem_sel + (size_t)warp * per_warp_bytes;
   double* qd = reinterpret_cast<double*>(base);                 // [D]
   float* work = reinterpret_cast<float*>(base + D * 8);         // [32][m + 4]
   int* sel = reinterpret_cast<int*>(work + 32 * stride);        // [32]
 
-  const int j = unit % n_b;
-  const size_t slice = unit / n_b;  // b * Hkv + kv
+  const int j = jb + widx % nj;          // blocks [jb, jb + nj) of every slice
+  const size_t slice = widx / nj;        // b * Hkv + kv
+  const size_t unit = slice * n_b + j;   // row of every [B, Hkv, n_b, ...] table
   const float* row = scores + (size_t)unit * n_b;
   const int lo = F, hi = j - L_eff;
   const int n = hi > lo ? hi - lo : 0;
@@ -418,10 +421,10 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
   const int nt = (d.n_b + kTile - 1) / kTile;
   dim3 grid(nt * (nt + 1) / 2, d.Hkv, d.B);
-  score_kernel<<<grid, 64, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff);
+  score_kernel<<<grid, 64, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff, d.jb, d.jb + d.nj);
   if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
 
-  const int n_units = d.B * d.Hkv * d.n_b;
+  const int n_units = d.B * d.Hkv * d.nj;
   const int kc_cap = d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b;
   if (d.Kc <= 32 && kc_cap * d.gpc <= 128) {
     // fast path: register/redux rounds, one candidate per lane in the group stage
@@ -437,7 +440,7 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
       HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
                                                                    n_chunks, group_idx, group_score, n_groups, n_units,
-                                                                   d.n_b, d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, lm,
+                                                                   d.jb, d.nj, d.n_b, d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, lm,
                                                                    per_warp_bytes);
       return launch_status();
     }
@@ -450,7 +453,7 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
   auto kern = d.D == 128 ? select_generic_kernel<128> : select_generic_kernel<64>;
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
-                                                               n_chunks, group_idx, group_score, n_groups, n_units, d.n_b,
+                                                               n_chunks, group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b,
                                                                d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp);
   return launch_status();
 }

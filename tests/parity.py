@@ -150,7 +150,7 @@ def check_against_oracle(w: W.Workload, q, k, v, p, buf, slices, blocks, check_i
     return rep
 
 
-def assert_report(rep, w: W.Workload, n_checked: int):
+def assert_report(rep, w: W.Workload, n_checked: int, score_tol: float = 1e-6):
     wst, tol = rep["worst"], rep["tol"]
     assert rep["chunk"]["bad"] == 0 and rep["group"]["bad"] == 0, rep
     # ties within 1e-6 relative must be rare
@@ -158,6 +158,6 @@ def assert_report(rep, w: W.Workload, n_checked: int):
     assert wst["out"] <= tol, rep
     assert wst["lse"] <= (1e-4 if w.dtype == "f32" else 2e-2), rep
     assert wst["pooled"] <= 2e-6 and wst["chunk_sum"] <= 2e-6 and wst["group_sum"] <= 4e-6, rep
-    assert wst["score"] <= 1e-6, rep
+    assert wst["score"] <= score_tol, rep
     # rotated keys: one storage rounding apart at most (fp32: ~1e-6 abs; bf16: 1 ulp of values up to ~8 -> 2^-4)
     assert wst["k_rot"] <= (4e-6 if w.dtype == "f32" else 0.0625), rep

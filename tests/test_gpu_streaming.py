@@ -1,0 +1,140 @@
+"""GPU parity tests (-m gpu) of the streaming step hga_prefill_window: chunk-by-chunk prefill,
+ragged prompt tail and single-token decode through the C ABI against the oracle's hga_oracle_step, which is handed only
+the history a step may see.  PAPER.md:158 (store/router cycle), :281 and Table 7 :291-292 ("vectorized prefill and
+chunk-by-chunk decode must agree up to floating-point noise").
+
+Every cache tensor starts as NaN (ints as -7) and rows are copied in only when their step arrives, so any read of the
+future shows up as a NaN in the result.
+"""
+import numpy as np
+import pytest
+import torch
+
+import hga_workloads as W
+import oracle
+import paper_2606_30709_b200 as hga
+from paper_2606_30709_b200.binding import ATTEND_AUTO, ATTEND_SIMT, HGA_F32, PrefillBuffers
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+BF16_W = W.Workload("stream_bf16", 2, 1280, 8, 2, 128, "bf16", 1.0e6, topk_chunks=3, topk_groups=8, n_clusters=4)
+F32_W = W.Workload("stream_f32", 1, 1024, 4, 1, 64, "f32", 1.0e4, topk_chunks=4, topk_groups=8, dist="iid")
+
+
+def _poisoned_cache(w, p):
+    dt = torch.bfloat16 if w.dtype == "bf16" else torch.float32
+    live = [torch.full((w.batch, h, w.seq, w.head_dim), float("nan"), dtype=dt, device="cuda")
+            for h in (w.n_q_heads, w.n_kv_heads, w.n_kv_heads)]
+    buf = PrefillBuffers.allocate(p)
+    for name in ("q_rot", "k_rot", "q_pooled", "chunk_sum", "group_sum", "chunk_score", "group_score", "out", "lse"):
+        getattr(buf, name).fill_(float("nan"))
+    for name in ("chunk_idx", "n_chunks", "group_idx", "n_groups"):
+        getattr(buf, name).fill_(-7)
+    return live, buf
+
+
+def _feed(live, full, t0, t1):
+    for dst, src in zip(live, full):
+        dst[:, :, t0:t1] = src[:, :, t0:t1]
+
+
+@pytest.mark.parametrize("w", [BF16_W, F32_W], ids=lambda w: w.name)
+def test_chunk_by_chunk_equals_vectorised_prefill(w):
+    q, k, v = W.generate(w, 3)
+    p = hga.params_from_workload(w)
+    full = parity.to_device(w, (q, k, v))
+    ref = hga.hga_prefill(p, *full)
+    live, buf = _poisoned_cache(w, p)
+    for j in range(w.n_blocks):
+        _feed(live, full, j * 64, (j + 1) * 64)
+        hga.hga_prefill_window(p, *live, buf, j * 64, (j + 1) * 64)
+    torch.cuda.synchronize()
+    # same kernels, same arithmetic order: the two modes agree bit for bit, not just "up to floating-point noise"
+    for name in ("q_rot", "k_rot", "q_pooled", "chunk_sum", "group_sum", "chunk_idx", "n_chunks", "group_idx", "n_groups",
+                 "out", "lse"):
+        a, b = getattr(buf, name), getattr(ref, name)
+        assert torch.equal(a, b), name
+    assert bool(torch.isfinite(buf.out).all())
+    # and the streamed result against the oracle
+    slices = [(b, kh) for b in range(w.batch) for kh in range(w.n_kv_heads)]
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, slices, np.arange(w.n_blocks))
+    # scores: the GPU dots fp32-STORED q_pooled and summaries (2^-24 relative each, reading R7), so the error scales with
+    # |q||s|; with at most 18 candidates per row the row's max |score| can sit well below that, hence 4e-6 here
+    parity.assert_report(rep, w, w.n_blocks * len(slices), score_tol=4e-6)
+
+
+def _check_step(w, op, q, k, v, buf, t0, t1, tol):
+    """Rows [t0, t1) of the GPU cache against oracle.step on every (batch, kv head) slice."""
+    G, j = op.G, t0 // 64
+    worst = 0.0
+    for b in range(w.batch):
+        for kh in range(w.n_kv_heads):
+            r = oracle.step(op, q[b, kh * G:(kh + 1) * G, t0:t1], k[b, kh, :t1], v[b, kh, :t1], t0, t1)
+            assert buf.n_chunks[b, kh, j].item() == r.n_chunks and buf.n_groups[b, kh, j].item() == r.n_groups
+            assert np.array_equal(buf.chunk_idx[b, kh, j].cpu().numpy()[:op.Kc], r.chunk_idx), (b, kh, t0, t1)
+            assert np.array_equal(buf.group_idx[b, kh, j].cpu().numpy()[:op.Kg], r.group_idx), (b, kh, t0, t1)
+            assert np.abs(buf.q_pooled[b, kh, j].cpu().numpy() - r.q_pooled).max() <= 2e-6
+            got = buf.out[b, kh * G:(kh + 1) * G, t0:t1].float().cpu().numpy().astype(np.float64)
+            lse = buf.lse[b, kh * G:(kh + 1) * G, t0:t1].cpu().numpy().astype(np.float64)
+            assert np.isfinite(got).all() and np.isfinite(lse).all()
+            worst = max(worst, float(np.abs(got - r.out).max()), float(np.abs(lse - r.lse).max()))
+    assert worst <= tol, (t0, t1, worst)
+    return worst
+
+
+@pytest.mark.parametrize("w,impl", [(BF16_W, ATTEND_AUTO), (BF16_W, ATTEND_SIMT), (F32_W, ATTEND_AUTO)],
+                         ids=["bf16_tc", "bf16_simt", "f32"])
+def test_ragged_prefill_then_decode_matches_oracle_step(w, impl):
+    """Prefill a ragged prompt (T0 not a multiple of 64) in one call, then decode token by token across a chunk
+    boundary, then a partial-chunk append and a decode step that can route to the chunk closed during decode."""
+    q, k, v = W.generate(w, 5)
+    p = hga.params_from_workload(w, attend_impl=impl)
+    op = oracle.params_from_workload(w)
+    tol = parity.TOL_OUT[w.dtype]
+    full = parity.to_device(w, (q, k, v))
+    live, buf = _poisoned_cache(w, p)
+    T0 = 13 * 64 + 40  # 872
+    _feed(live, full, 0, T0)
+    hga.hga_prefill_window(p, *live, buf, 0, T0)
+    torch.cuda.synchronize()
+    for j in (0, 1, 2, 5, 9, 12):
+        _check_step(w, op, q, k, v, buf, j * 64, (j + 1) * 64, tol)
+    _check_step(w, op, q, k, v, buf, 13 * 64, T0, tol)  # the ragged tail block
+    # decode across the boundary at 896: the step of token 895 closes chunk 13 and writes its summaries
+    for t in range(T0, 905):
+        _feed(live, full, t, t + 1)
+        hga.hga_prefill_window(p, *live, buf, t, t + 1)
+        torch.cuda.synchronize()
+        _check_step(w, op, q, k, v, buf, t, t + 1, tol)
+    # partial-chunk append inside chunk 14, then the rest of it
+    for (a, b) in ((905, 930), (930, 960)):
+        _feed(live, full, a, b)
+        hga.hga_prefill_window(p, *live, buf, a, b)
+        torch.cuda.synchronize()
+        _check_step(w, op, q, k, v, buf, a, b, tol)
+    # decode in chunk 15: chunk 13 (closed during decode) is now a middle candidate
+    _feed(live, full, 960, 961)
+    hga.hga_prefill_window(p, *live, buf, 960, 961)
+    torch.cuda.synchronize()
+    _check_step(w, op, q, k, v, buf, 960, 961, tol)
+    # the summaries written by the streaming steps equal a vectorised pass over the closed chunks
+    ref = hga.hga_prefill(p, *full)
+    torch.cuda.synchronize()
+    assert torch.equal(buf.chunk_sum[:, :, :15], ref.chunk_sum[:, :, :15])
+    assert torch.equal(buf.group_sum[:, :, :60], ref.group_sum[:, :, :60])
+    assert torch.equal(buf.k_rot[:, :, :961], ref.k_rot[:, :, :961])
+    assert bool(torch.isnan(buf.k_rot[:, :, 961:].float()).all())  # nothing past the last step was written
+
+
+def test_window_argument_errors():
+    w = F32_W
+    p = hga.params_from_workload(w)
+    q, k, v = parity.to_device(w, W.generate(w, 0))
+    buf = PrefillBuffers.allocate(p)
+    for (a, b) in ((10, 70), (0, 0), (5, 4), (-1, 3), (0, w.seq + 1), (w.seq, w.seq + 1)):
+        with pytest.raises(RuntimeError, match="HGA_ERR_INVALID_ARG"):
+            hga.hga_prefill_window(p, q, k, v, buf, a, b)
+    hga.hga_prefill_window(p, q, k, v, buf, 64, 64 + 70)  # starts on a boundary: may span blocks and end ragged
+    torch.cuda.synchronize()
