@@ -30,6 +30,11 @@ class Workload:
     n_clusters: int = 32
     cluster_scale: float = 2.0
     pos0: int = 0
+    n_valid: int = 0  # prompt tokens actually present (ragged tail); 0 = seq.  `seq` is then the cache capacity
+
+    @property
+    def n_tokens(self) -> int:
+        return self.n_valid if self.n_valid > 0 else self.seq
 
     @property
     def n_blocks(self) -> int:
@@ -54,6 +59,11 @@ CONFIGS = {
     "c3": Workload("c3", 8, 12288, 8, 8, 64, "bf16", 1.0e4, topk_chunks=16, topk_groups=32),
     "c4": Workload("c4", 1, 32768, 32, 4, 128, "bf16", 1.0e6, topk_chunks=16, topk_groups=64),
     "c5": Workload("c5", 1, 65536, 32, 4, 128, "bf16", 1.0e6, topk_chunks=12, topk_groups=48),
+    # the paper's own needle-test parameters: 65,599 prompt tokens across
+    # 1,025 chunks (a ragged last chunk of 63 tokens), keep first 2 / keep last 8, K_c = 20, K_g = 32 (group refinement
+    # keeps 32 of 80 candidate groups), Qwen3-30B-A3B head shape.  Attended: 32*16 + 11*64 = 1216 tokens = 1.85 %.
+    "p5": Workload("p5", 1, 65600, 32, 4, 128, "bf16", 1.0e6, n_sink=2, n_local=8, topk_chunks=20, topk_groups=32,
+                   n_valid=65599),
 }
 
 

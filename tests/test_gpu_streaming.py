@@ -138,3 +138,49 @@ def test_window_argument_errors():
             hga.hga_prefill_window(p, q, k, v, buf, a, b)
     hga.hga_prefill_window(p, q, k, v, buf, 64, 64 + 70)  # starts on a boundary: may span blocks and end ragged
     torch.cuda.synchronize()
+
+
+def test_paper_needle_parameters_ragged_64k_p5():
+    """the paper's own 64K needle-test parameters at full size -- 65,599
+    prompt tokens across 1,025 chunks (ragged last chunk of 63 tokens), keep first 2 / keep last 8, K_c = 20 refined to
+    K_g = 32 of 80 candidate groups, Qwen3 head shape -- in one hga_prefill_window call, on sampled blocks."""
+    w = W.get("p5")
+    assert (w.n_tokens, w.n_blocks) == (65599, 1025)
+    q, k, v = W.generate(w, 0)
+    p = hga.params_from_workload(w)
+    op = oracle.params_from_workload(w)
+    full = parity.to_device(w, (q, k, v))
+    live, buf = _poisoned_cache(w, p)
+    _feed(live, full, 0, w.n_tokens)
+    hga.hga_prefill_window(p, *live, buf, 0, w.n_tokens)
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev[0].record()
+    for _ in range(5):
+        hga.hga_prefill_window(p, *live, buf, 0, w.n_tokens)
+    ev[1].record()
+    torch.cuda.synchronize()
+    print(f"p5 hga_prefill_window(0, 65599): {ev[0].elapsed_time(ev[1]) / 5:.3f} ms per call")
+    # budgets: every steady-state block opens exactly K_g = 32 groups -> 32*16 + (2+8+1)*64 = 1216 attended tokens,
+    # the paper's "approximately 1.9% sparsity" (1216 / 65599 = 1.85 %)
+    ng = buf.n_groups.cpu().numpy()
+    nc = buf.n_chunks.cpu().numpy()
+    jj = np.arange(w.n_blocks)
+    assert np.all(nc == np.minimum(20, np.maximum(0, jj - 10))[None, None])
+    assert np.all(ng == np.minimum(32, 4 * nc))
+    assert bool(torch.isfinite(buf.out[:, :, :w.n_tokens]).all())
+    assert bool(torch.isnan(buf.out[:, :, w.n_tokens:]).all())  # the padding row of the cache is never written
+    # sampled blocks on two slices against the oracle step (handed only the prefix)
+    class _One:  # restrict _check_step to one slice
+        batch, n_kv_heads = 1, 1
+    G = op.G
+    for kh in (0, 3):
+        sl = (slice(0, 1), slice(kh, kh + 1))
+        qs, ks, vs = q[:, kh * G:(kh + 1) * G], k[sl], v[sl]
+        view = type("B", (), {n: getattr(buf, n)[:, kh:kh + 1] for n in
+                              ("n_chunks", "n_groups", "chunk_idx", "group_idx", "q_pooled")})
+        view.out = buf.out[:, kh * G:(kh + 1) * G]
+        view.lse = buf.lse[:, kh * G:(kh + 1) * G]
+        for j in (0, 3, 10, 11, 12, 31, 500 + kh, 1023):
+            _check_step(_One, op, qs, ks, vs, view, j * 64, (j + 1) * 64, parity.TOL_OUT["bf16"])
+        _check_step(_One, op, qs, ks, vs, view, 1024 * 64, w.n_tokens, parity.TOL_OUT["bf16"])  # ragged tail block
