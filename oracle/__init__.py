@@ -13,6 +13,7 @@ from .hga_oracle import (  # noqa: F401
     dense_block,
     key_set,
     max_threads,
+    n_hi_rule,
     params_from_workload,
     pool_queries,
     prefill,

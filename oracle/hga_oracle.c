@@ -56,6 +56,10 @@ typedef struct {
   int64_t pos0;       /* position of token 0 */
   double base;        /* RoPE base */
   double scale;       /* softmax scale; <= 0 -> 1/sqrt(D) (Eq. 1) */
+  int64_t pos_mod;    /* N3 variant: RoPE position index wrapped, p <- p mod pos_mod (the paper uses
+                         65536); 0 = off.  Reading R18: every position that enters a rotation is wrapped, and
+                         pos_mod and pos0 must be multiples of C so that no span straddles a wrap (its "middle
+                         position" R2 is then wrapped start + (S-1)/2); the routing algorithm is unchanged. */
 } hga_oracle_params;
 
 int hga_oracle_max_threads(void) {
@@ -78,12 +82,16 @@ static void rot_pair(double a, double b, double ang, double* oa, double* ob) {
   *ob = b * c + a * s;
 }
 
-/* x [n_rows, D] fp32; row r sits at position pos_first + r.  out [n_rows, D] fp64. */
-int hga_oracle_rope(const float* x, int n_rows, int D, int64_t pos_first, double base, double* out) {
-  if (D <= 0 || (D & 1)) return HGA_ORACLE_ERR_ARG;
+/* N3: the position index that enters a rotation, p <- p mod pos_mod; pos_mod = 0 leaves p as is */
+static int64_t wrap_pos(int64_t p, int64_t pos_mod) { return pos_mod > 0 ? p % pos_mod : p; }
+
+/* x [n_rows, D] fp32; row r sits at position pos_first + r (wrapped modulo pos_mod if > 0).  out [n_rows, D] fp64. */
+int hga_oracle_rope_mod(const float* x, int n_rows, int D, int64_t pos_first, int64_t pos_mod, double base,
+                        double* out) {
+  if (D <= 0 || (D & 1) || pos_mod < 0 || pos_first < 0) return HGA_ORACLE_ERR_ARG;
   int half = D / 2;
   for (int r = 0; r < n_rows; ++r) {
-    double p = (double)(pos_first + r);
+    double p = (double)wrap_pos(pos_first + r, pos_mod);
     for (int i = 0; i < half; ++i) {
       double th = hga_oracle_theta(D, base, i);
       rot_pair((double)x[(size_t)r * D + i], (double)x[(size_t)r * D + i + half], p * th,
@@ -91,6 +99,10 @@ int hga_oracle_rope(const float* x, int n_rows, int D, int64_t pos_first, double
     }
   }
   return HGA_ORACLE_OK;
+}
+
+int hga_oracle_rope(const float* x, int n_rows, int D, int64_t pos_first, double base, double* out) {
+  return hga_oracle_rope_mod(x, n_rows, D, pos_first, 0, base, out);
 }
 
 /* Storage rounding R7: round fp64 -> nearest fp32, or nearest bf16 (ties to even), in ONE rounding. */
@@ -117,16 +129,33 @@ int hga_oracle_default_n_hi(int D, double base, int span) {
   return n;
 }
 
+/* N3 variants of R1 (the paper gives no threshold): which pairs are "high-frequency" for a span of
+   S tokens.  rule 0: wavelength 2*pi/theta_i <= S (the default above); rule 1: the span sweeps at least half a turn,
+   theta_i * S >= pi; rule 2: the span sweeps at least one radian, theta_i * S >= 1.  theta_i decreases with i, so
+   each rule selects a leading block of pairs and the count is all a caller needs (passed as n_hi). */
+int hga_oracle_n_hi_rule(int D, double base, int span, int rule) {
+  int n = 0;
+  for (int i = 0; i < D / 2; ++i) {
+    double th = hga_oracle_theta(D, base, i);
+    int hi = rule == 0 ? (2.0 * M_PI / th <= (double)span)
+           : rule == 1 ? (th * (double)span >= M_PI)
+           : rule == 2 ? (th * (double)span >= 1.0) : 0;
+    if (hi) ++n;
+  }
+  return (rule < 0 || rule > 2) ? -1 : n;
+}
+
 /* k_raw [N,D] fp32 (un-rotated keys); spans of S tokens; out [N/S, D] fp64. */
-int hga_oracle_summaries(const float* k_raw, int N, int D, int S, int n_hi, int64_t pos0, double base,
-                         double* out) {
-  if (S <= 0 || N % S || (D & 1)) return HGA_ORACLE_ERR_ARG;
+int hga_oracle_summaries_mod(const float* k_raw, int N, int D, int S, int n_hi, int64_t pos0, int64_t pos_mod,
+                             double base, double* out) {
+  if (S <= 0 || N % S || (D & 1) || pos_mod < 0 || pos0 < 0) return HGA_ORACLE_ERR_ARG;
+  if (pos_mod > 0 && (pos_mod % S || pos0 % S)) return HGA_ORACLE_ERR_ARG; /* R18: no span straddles a wrap */
   int half = D / 2;
   if (n_hi < 0) n_hi = hga_oracle_default_n_hi(D, base, S);
   if (n_hi > half) return HGA_ORACLE_ERR_ARG;
   for (int sp = 0; sp < N / S; ++sp) {
     int start = sp * S;
-    double p_mid = (double)pos0 + (double)start + 0.5 * (double)(S - 1);
+    double p_mid = (double)wrap_pos(pos0 + start, pos_mod) + 0.5 * (double)(S - 1);
     for (int i = 0; i < half; ++i) {
       double th = hga_oracle_theta(D, base, i);
       double sa = 0.0, sb = 0.0;
@@ -135,7 +164,8 @@ int hga_oracle_summaries(const float* k_raw, int N, int D, int S, int n_hi, int6
         for (int t = 0; t < S; ++t) {
           double ra, rb;
           const float* row = k_raw + (size_t)(start + t) * D;
-          rot_pair((double)row[i], (double)row[i + half], (double)(pos0 + start + t) * th, &ra, &rb);
+          rot_pair((double)row[i], (double)row[i + half], (double)wrap_pos(pos0 + start + t, pos_mod) * th,
+                   &ra, &rb);
           sa += ra;
           sb += rb;
         }
@@ -158,6 +188,11 @@ int hga_oracle_summaries(const float* k_raw, int N, int D, int S, int n_hi, int6
     }
   }
   return HGA_ORACLE_OK;
+}
+
+int hga_oracle_summaries(const float* k_raw, int N, int D, int S, int n_hi, int64_t pos0, double base,
+                         double* out) {
+  return hga_oracle_summaries_mod(k_raw, N, D, S, n_hi, pos0, 0, base, out);
 }
 
 /* ------------------------------------------------------------------------------------------------ */
@@ -431,12 +466,12 @@ int hga_oracle_slice(const hga_oracle_params* p, const float* q_raw, const float
   int rc = HGA_ORACLE_OK;
   /* O1 keys */
   double* k_rot = (double*)malloc(sizeof(double) * (size_t)N * D);
-  rc |= hga_oracle_rope(k_raw, N, D, p->pos0, p->base, k_rot);
+  rc |= hga_oracle_rope_mod(k_raw, N, D, p->pos0, p->pos_mod, p->base, k_rot);
   /* O2 summaries from the RAW keys (the rule itself rotates), before any storage rounding (R7) */
   double* S_c = (double*)malloc(sizeof(double) * (size_t)n_b * D);
   double* S_g = (double*)malloc(sizeof(double) * (size_t)n_g * D);
-  rc |= hga_oracle_summaries(k_raw, N, D, C, p->n_hi_chunk, p->pos0, p->base, S_c);
-  rc |= hga_oracle_summaries(k_raw, N, D, gs, p->n_hi_group, p->pos0, p->base, S_g);
+  rc |= hga_oracle_summaries_mod(k_raw, N, D, C, p->n_hi_chunk, p->pos0, p->pos_mod, p->base, S_c);
+  rc |= hga_oracle_summaries_mod(k_raw, N, D, gs, p->n_hi_group, p->pos0, p->pos_mod, p->base, S_g);
   /* storage rounding of K_rot for O6 (R7) */
   hga_oracle_round_io(k_rot, (size_t)N * D, p->io_bf16);
   double* vd = (double*)malloc(sizeof(double) * (size_t)N * D);
@@ -457,8 +492,8 @@ int hga_oracle_slice(const hga_oracle_params* p, const float* q_raw, const float
     /* O1 queries of block j: q_blk [G,C,D] */
     double* q_blk = (double*)malloc(sizeof(double) * (size_t)G * C * D);
     for (int h = 0; h < G; ++h)
-      hga_oracle_rope(q_raw + ((size_t)h * N + (size_t)j * C) * D, C, D, p->pos0 + (int64_t)j * C, p->base,
-                      q_blk + (size_t)h * C * D);
+      hga_oracle_rope_mod(q_raw + ((size_t)h * N + (size_t)j * C) * D, C, D, p->pos0 + (int64_t)j * C, p->pos_mod,
+                          p->base, q_blk + (size_t)h * C * D);
     /* O3 pooled query from the un-rounded rotated queries (R7) */
     double* qbar = (double*)malloc(sizeof(double) * (size_t)D);
     hga_oracle_pool_queries(q_blk, G, C, D, C, qbar); /* a [G,C,D] tensor is one block of length C */
@@ -541,16 +576,17 @@ int hga_oracle_step(const hga_oracle_params* p, const float* q_win, const float*
   int* cidx = (int*)malloc(sizeof(int) * (size_t)(p->Kc > 0 ? p->Kc : 1));
   int* gidx = (int*)malloc(sizeof(int) * (size_t)(p->Kg > 0 ? p->Kg : 1));
   /* O1 keys of the visible history, O2 summaries of the closed chunks (from RAW keys, R7) */
-  rc |= hga_oracle_rope(k_raw, n_hist, D, p->pos0, p->base, k_rot);
+  rc |= hga_oracle_rope_mod(k_raw, n_hist, D, p->pos0, p->pos_mod, p->base, k_rot);
   if (n_closed > 0) {
-    rc |= hga_oracle_summaries(k_raw, n_closed * C, D, C, p->n_hi_chunk, p->pos0, p->base, S_c);
-    rc |= hga_oracle_summaries(k_raw, n_closed * C, D, gs, p->n_hi_group, p->pos0, p->base, S_g);
+    rc |= hga_oracle_summaries_mod(k_raw, n_closed * C, D, C, p->n_hi_chunk, p->pos0, p->pos_mod, p->base, S_c);
+    rc |= hga_oracle_summaries_mod(k_raw, n_closed * C, D, gs, p->n_hi_group, p->pos0, p->pos_mod, p->base, S_g);
   }
   hga_oracle_round_io(k_rot, (size_t)n_hist * D, p->io_bf16);
   for (size_t i = 0; i < (size_t)n_hist * D; ++i) vd[i] = (double)v[i];
   /* O1 window queries, O3 over the window (R17) */
   for (int h = 0; h < G; ++h)
-    rc |= hga_oracle_rope(q_win + (size_t)h * W * D, W, D, p->pos0 + t0, p->base, q_rot + (size_t)h * W * D);
+    rc |= hga_oracle_rope_mod(q_win + (size_t)h * W * D, W, D, p->pos0 + t0, p->pos_mod, p->base,
+                              q_rot + (size_t)h * W * D);
   rc |= hga_oracle_pool_queries(q_rot, G, W, D, W, qbar); /* a [G,W,D] tensor is one block of length W */
   if (rc) goto done;
   if (q_pooled) memcpy(q_pooled, qbar, sizeof(double) * (size_t)D);

@@ -33,7 +33,7 @@ class _Params(C.Structure):
         ("G", C.c_int32), ("N", C.c_int32), ("D", C.c_int32), ("C", C.c_int32), ("gs", C.c_int32),
         ("F", C.c_int32), ("L", C.c_int32), ("Kc", C.c_int32), ("Kg", C.c_int32),
         ("n_hi_chunk", C.c_int32), ("n_hi_group", C.c_int32), ("io_bf16", C.c_int32),
-        ("pos0", C.c_int64), ("base", C.c_double), ("scale", C.c_double),
+        ("pos0", C.c_int64), ("base", C.c_double), ("scale", C.c_double), ("pos_mod", C.c_int64),
     ]
 
 
@@ -54,16 +54,19 @@ class OracleParams:
     pos0: int = 0
     base: float = 1.0e4
     scale: float = 0.0
+    pos_mod: int = 0  # N3: RoPE position index wrapped modulo pos_mod; 0 = off
 
     def c_struct(self) -> _Params:
         return _Params(self.G, self.N, self.D, self.C, self.gs, self.F, self.L, self.Kc, self.Kg,
-                       self.n_hi_chunk, self.n_hi_group, int(self.io_bf16), self.pos0, self.base, self.scale)
+                       self.n_hi_chunk, self.n_hi_group, int(self.io_bf16), self.pos0, self.base, self.scale,
+                       self.pos_mod)
 
 
 def params_from_workload(w) -> OracleParams:
     return OracleParams(G=w.n_q_heads // w.n_kv_heads, N=w.seq, D=w.head_dim, C=w.chunk, gs=w.group, F=w.n_sink,
                         L=w.n_local, Kc=w.topk_chunks, Kg=w.topk_groups, io_bf16=(w.dtype == "bf16"),
-                        pos0=w.pos0, base=w.rope_base)
+                        pos0=w.pos0, base=w.rope_base, pos_mod=getattr(w, "rope_pos_mod", 0),
+                        n_hi_chunk=getattr(w, "n_hi_chunk", -1), n_hi_group=getattr(w, "n_hi_group", -1))
 
 
 def _L():
@@ -105,8 +108,17 @@ def default_n_hi(D: int, base: float, span: int) -> int:
     return int(_L().hga_oracle_default_n_hi(C.c_int(D), C.c_double(base), C.c_int(span)))
 
 
-def rope(x, pos_first: int, base: float) -> np.ndarray:
-    """x [..., n_rows, D] fp32, consecutive positions from pos_first along axis -2 -> fp64."""
+def n_hi_rule(D: int, base: float, span: int, rule: int) -> int:
+    """N3: # of leading high-frequency pairs under rule 0 (wavelength <= span), 1 (sweep >= pi), 2 (sweep >= 1 rad)."""
+    n = int(_L().hga_oracle_n_hi_rule(C.c_int(D), C.c_double(base), C.c_int(span), C.c_int(rule)))
+    if n < 0:
+        raise ValueError("unknown n_hi rule")
+    return n
+
+
+def rope(x, pos_first: int, base: float, pos_mod: int = 0) -> np.ndarray:
+    """x [..., n_rows, D] fp32, consecutive positions from pos_first along axis -2 (wrapped modulo pos_mod if > 0,
+    PAPER.md:259-264) -> fp64."""
     x = _f32(x)
     D = x.shape[-1]
     n_rows = x.shape[-2]
@@ -114,8 +126,8 @@ def rope(x, pos_first: int, base: float) -> np.ndarray:
     xf = x.reshape(-1, n_rows, D)
     of = out.reshape(-1, n_rows, D)
     for i in range(xf.shape[0]):
-        _check(_L().hga_oracle_rope(_p(xf[i], C.c_float), C.c_int(n_rows), C.c_int(D), C.c_int64(pos_first),
-                                    C.c_double(base), _p(of[i], C.c_double)), "rope")
+        _check(_L().hga_oracle_rope_mod(_p(xf[i], C.c_float), C.c_int(n_rows), C.c_int(D), C.c_int64(pos_first),
+                                        C.c_int64(pos_mod), C.c_double(base), _p(of[i], C.c_double)), "rope")
     return out
 
 
@@ -125,13 +137,14 @@ def round_io(x, io_bf16: bool) -> np.ndarray:
     return out
 
 
-def summaries(k_raw, span: int, n_hi: int, pos0: int, base: float) -> np.ndarray:
+def summaries(k_raw, span: int, n_hi: int, pos0: int, base: float, pos_mod: int = 0) -> np.ndarray:
     """k_raw [N,D] fp32 -> [N/span, D] fp64 mixed-RoPE summaries."""
     k_raw = _f32(k_raw)
     N, D = k_raw.shape
     out = np.empty((N // span, D), dtype=np.float64)
-    _check(_L().hga_oracle_summaries(_p(k_raw, C.c_float), C.c_int(N), C.c_int(D), C.c_int(span), C.c_int(n_hi),
-                                     C.c_int64(pos0), C.c_double(base), _p(out, C.c_double)), "summaries")
+    _check(_L().hga_oracle_summaries_mod(_p(k_raw, C.c_float), C.c_int(N), C.c_int(D), C.c_int(span), C.c_int(n_hi),
+                                         C.c_int64(pos0), C.c_int64(pos_mod), C.c_double(base),
+                                         _p(out, C.c_double)), "summaries")
     return out
 
 

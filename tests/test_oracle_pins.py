@@ -550,3 +550,91 @@ def test_c5_needle_group_is_routed_by_the_oracle():
         r0 = oracle.prefill_slice(op, q[0, kh * G:(kh + 1) * G], k[0, kh], v[0, kh], blocks=[w.n_blocks - 1],
                                   attend=False, want_k_rot=False)
         assert g_star not in r0.group_idx[0]
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# N3 variants: wrapped RoPE position index and alternative high-frequency thresholds (R1)
+# ----------------------------------------------------------------------------------------------------------------
+def test_rope_position_wrap_matches_complex_rotation_at_wrapped_positions():
+    M = int(golden()["rope_wrap_modulus"])
+    assert M == 65536
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal((192, 32)).astype(np.float32)
+    # rows straddle the wrap: positions M-64 .. M+127 become M-64 .. M-1, 0 .. 127
+    got = oracle.rope(x, M - 64, 1.0e4, pos_mod=M)
+    pos = (np.arange(M - 64, M + 128) % M)
+    assert np.abs(got - rope_complex(x, pos, 1.0e4)).max() < 1e-9
+    # after the wrap the rotation is the un-wrapped rotation of position p - M (periodicity of the index, not of RoPE)
+    assert np.array_equal(got[64:], oracle.rope(x[64:], 0, 1.0e4))
+    # a modulus no position reaches changes nothing, bit for bit
+    assert np.array_equal(oracle.rope(x, 100, 1.0e4, pos_mod=M), oracle.rope(x, 100, 1.0e4))
+    # and wrapping is NOT the identity: the pair with theta = 1 (i = 0) differs at position M vs 0 unless M*1 = 2*pi*k
+    assert np.abs(got[64:] - oracle.rope(x[64:], M, 1.0e4)).max() > 1e-2
+
+
+def test_summaries_under_position_wrap():
+    w, q, k, v = small_problem(4, N=256, D=32)
+    M = 128  # spans 0,1 sit at positions 64..127, spans 2,3 wrap to 0..127 (pos0 = 64)
+    pos = (64 + np.arange(256)) % M
+    for span in (64, 16):
+        # all pairs high: mean of the keys rotated at their wrapped positions (P11 under the wrap)
+        s = oracle.summaries(k, span, 16, 64, w.rope_base, pos_mod=M)
+        assert np.abs(s - rope_complex(k, pos, w.rope_base).reshape(-1, span, 32).mean(1)).max() < 1e-12
+        # all pairs low: raw mean rotated at the wrapped start + (S-1)/2 (P12 under the wrap, reading R18)
+        s = oracle.summaries(k, span, 0, 64, w.rope_base, pos_mod=M)
+        p_mid = pos.reshape(-1, span)[:, 0] + (span - 1) / 2.0
+        raw_mean = k.astype(np.float64).reshape(-1, span, 32).mean(1)
+        assert np.abs(s - rope_complex(raw_mean, p_mid, w.rope_base)).max() < 1e-12
+    # a span may not straddle a wrap: modulus or pos0 off the span grid is rejected
+    with pytest.raises(Exception):
+        oracle.summaries(k, 64, 4, 0, w.rope_base, pos_mod=96)
+    with pytest.raises(Exception):
+        oracle.summaries(k, 64, 4, 32, w.rope_base, pos_mod=128)
+
+
+def test_prefill_under_position_wrap_is_a_global_shift_and_leaves_routing_unchanged():
+    w, q, k, v = small_problem(8, G=2, N=512, D=32, clustered=True)
+    base = dict(G=2, N=512, D=32, F=1, L=1, Kc=3, Kg=5, base=w.rope_base)
+    r_plain = oracle.prefill_slice(oracle.OracleParams(**base), q, k, v)
+    # a sequence that starts exactly at the modulus is position-for-position the sequence that starts at 0
+    r_wrap = oracle.prefill_slice(oracle.OracleParams(**base, pos0=1024, pos_mod=1024), q, k, v)
+    assert np.array_equal(r_plain.chunk_idx, r_wrap.chunk_idx) and np.array_equal(r_plain.group_idx, r_wrap.group_idx)
+    assert np.array_equal(r_plain.out, r_wrap.out)
+    # a modulus beyond the last position is inert
+    r_big = oracle.prefill_slice(oracle.OracleParams(**base, pos_mod=65536), q, k, v)
+    assert np.array_equal(r_plain.out, r_big.out) and np.array_equal(r_plain.group_idx, r_big.group_idx)
+    # a wrap in the middle of the sequence changes the logits (positions 256.. alias 0..) but the routing algorithm
+    # is "unchanged": same budgets, same visibility windows, still exact softmax over the union set
+    pw = oracle.OracleParams(**base, pos_mod=256)
+    r_mid = oracle.prefill_slice(pw, q, k, v)
+    assert np.array_equal(r_mid.n_chunks, r_plain.n_chunks) and np.array_equal(r_mid.n_groups, r_plain.n_groups)
+    assert np.abs(r_mid.out - r_plain.out).max() > 1e-3
+    # ... checked against a direct computation: rotate at wrapped positions, softmax over the oracle's own key set
+    pos = np.arange(512) % 256
+    qr = rope_complex(q, pos, w.rope_base)
+    kr = rope_complex(k, pos, w.rope_base)
+    j = 7
+    keys = oracle.key_set(j, 64, 16, 1, 1, r_mid.group_idx[j])
+    for t in (j * 64, j * 64 + 37, j * 64 + 63):
+        vis = np.flatnonzero(keys & (np.arange(keys.size) <= t))  # union set, causal cut inside the block
+        lg = (qr[1, t] @ kr[vis].T) / math.sqrt(32)
+        pr = np.exp(lg - lg.max())
+        ref = (pr / pr.sum()) @ v[vis].astype(np.float64)
+        assert np.abs(r_mid.out[j, 1, t - j * 64] - ref).max() < 1e-5  # Q_rot/K_rot are stored as fp32 (R7)
+
+
+def test_n_hi_rules_closed_form():
+    # theta_i = base^(-2i/D) decreases with i, so each rule keeps pairs i <= (D/2) ln(S/c) / ln(base):
+    # c = 2*pi (wavelength <= span), pi (half a turn), 1 (one radian)
+    for D, base in ((64, 1.0e4), (128, 1.0e6), (32, 100.0)):
+        for span in (64, 16):
+            for rule, c in ((0, 2 * math.pi), (1, math.pi), (2, 1.0)):
+                x = (D / 2) * math.log(span / c) / math.log(base)
+                want = min(D // 2, max(0, math.floor(x) + 1)) if x >= 0 else 0
+                assert oracle.n_hi_rule(D, base, span, rule) == want, (D, base, span, rule)
+            assert oracle.n_hi_rule(D, base, span, 0) == oracle.default_n_hi(D, base, span)
+    # the counts SURVEY.md 8(c) R1 lists for the two model shapes (chunk / group)
+    assert [oracle.n_hi_rule(64, 1e4, s, r) for r in range(3) for s in (64, 16)] == [9, 4, 11, 6, 15, 10]
+    assert [oracle.n_hi_rule(128, 1e6, s, r) for r in range(3) for s in (64, 16)] == [11, 5, 14, 8, 20, 13]
+    with pytest.raises(ValueError):
+        oracle.n_hi_rule(64, 1e4, 64, 3)
