@@ -85,6 +85,10 @@ typedef enum {
  *   (PAPER.md:84-87).  -1 selects the default: pairs whose wavelength 2*pi/theta_i is <= the span length.
  *   RoPE: pair i = (x[i], x[i + head_dim/2]), theta_i = rope_base^(-2i/head_dim), position of token t = pos0 + t.
  *   softmax_scale 0 -> 1/sqrt(head_dim) (Eq. 1).
+ *   rope_pos_mod (variant of PAPER.md:259-264, "p <- p mod 65536"): when > 0, every position that enters a rotation
+ *   (Q, K, both summary rules) is wrapped modulo it; the routing algorithm is unchanged.  It and pos0 must then be
+ *   multiples of `chunk`, so that no chunk or group straddles a wrap (its middle position is the wrapped start +
+ *   (S-1)/2); otherwise HGA_ERR_INVALID_ARG.  0 = off.
  */
 typedef struct hga_params {
   int32_t batch, seq, n_q_heads, n_kv_heads, head_dim;
@@ -98,7 +102,7 @@ typedef struct hga_params {
   int64_t pos0;
   double rope_base;
   float softmax_scale;
-  int32_t reserved;    /* must be 0 */
+  int32_t rope_pos_mod; /* 0 = off */
 } hga_params;
 
 HGA_API const char* hga_status_string(hga_status s);
@@ -108,6 +112,12 @@ HGA_API int32_t hga_version(void);
 
 /* Default high-frequency pair count for a span of `span` tokens (rule above).  Host arithmetic only. */
 HGA_API int32_t hga_default_n_hi(int32_t head_dim, double rope_base, int32_t span);
+
+/* Alternative thresholds for "high-frequency" (the paper gives none): the count of leading pairs for
+ * a span of `span` tokens under rule 0 (wavelength 2*pi/theta_i <= span, the default), 1 (the span sweeps at least
+ * half a turn: theta_i*span >= pi) or 2 (at least one radian: theta_i*span >= 1).  Pass the result as n_hi_chunk /
+ * n_hi_group.  Returns -1 for an unknown rule.  Host arithmetic only. */
+HGA_API int32_t hga_n_hi_rule(int32_t head_dim, double rope_base, int32_t span, int32_t rule);
 
 /* Validate `p` without touching the GPU. */
 HGA_API hga_status hga_validate(const hga_params* p);

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     hga_attend,
     hga_build_summaries,
     hga_default_n_hi,
+    hga_n_hi_rule,
     hga_prefill,
     hga_prefill_profile,
     hga_prefill_window,

@@ -29,7 +29,7 @@ class _CParams(C.Structure):
         ("head_dim", C.c_int32), ("chunk", C.c_int32), ("group", C.c_int32), ("n_sink", C.c_int32),
         ("n_local", C.c_int32), ("topk_chunks", C.c_int32), ("topk_groups", C.c_int32), ("n_hi_chunk", C.c_int32),
         ("n_hi_group", C.c_int32), ("io_dtype", C.c_int32), ("out_dtype", C.c_int32), ("attend_impl", C.c_int32),
-        ("pos0", C.c_int64), ("rope_base", C.c_double), ("softmax_scale", C.c_float), ("reserved", C.c_int32),
+        ("pos0", C.c_int64), ("rope_base", C.c_double), ("softmax_scale", C.c_float), ("rope_pos_mod", C.c_int32),
     ]
 
 
@@ -58,6 +58,8 @@ def load_library():
     lib.hga_version.restype = C.c_int32
     lib.hga_default_n_hi.restype = C.c_int32
     lib.hga_default_n_hi.argtypes = [C.c_int32, C.c_double, C.c_int32]
+    lib.hga_n_hi_rule.restype = C.c_int32
+    lib.hga_n_hi_rule.argtypes = [C.c_int32, C.c_double, C.c_int32, C.c_int32]
     lib.hga_validate.argtypes = [P]
     lib.hga_workspace_bytes.argtypes = [P, C.POINTER(C.c_size_t)]
     lib.hga_rope.argtypes = [P, V, I, V, F, V]
@@ -99,11 +101,13 @@ class Params:
     pos0: int = 0
     rope_base: float = 1.0e4
     softmax_scale: float = 0.0
+    rope_pos_mod: int = 0
 
     def c(self) -> _CParams:
         return _CParams(self.batch, self.seq, self.n_q_heads, self.n_kv_heads, self.head_dim, self.chunk, self.group,
                         self.n_sink, self.n_local, self.topk_chunks, self.topk_groups, self.n_hi_chunk, self.n_hi_group,
-                        self.io_dtype, self.out_dtype, self.attend_impl, self.pos0, self.rope_base, self.softmax_scale, 0)
+                        self.io_dtype, self.out_dtype, self.attend_impl, self.pos0, self.rope_base, self.softmax_scale,
+                        self.rope_pos_mod)
 
     @property
     def n_blocks(self) -> int:
@@ -125,7 +129,9 @@ def params_from_workload(w, out_dtype: int = HGA_F32, attend_impl: int = ATTEND_
     return Params(batch=w.batch, seq=w.seq, n_q_heads=w.n_q_heads, n_kv_heads=w.n_kv_heads, head_dim=w.head_dim,
                   chunk=w.chunk, group=w.group, n_sink=w.n_sink, n_local=w.n_local, topk_chunks=w.topk_chunks,
                   topk_groups=w.topk_groups, io_dtype=HGA_BF16 if w.dtype == "bf16" else HGA_F32, out_dtype=out_dtype,
-                  attend_impl=attend_impl, pos0=w.pos0, rope_base=w.rope_base)
+                  attend_impl=attend_impl, pos0=w.pos0, rope_base=w.rope_base,
+                  n_hi_chunk=getattr(w, "n_hi_chunk", -1), n_hi_group=getattr(w, "n_hi_group", -1),
+                  rope_pos_mod=getattr(w, "rope_pos_mod", 0))
 
 
 def _check(code: int, what: str):
@@ -150,6 +156,10 @@ def hga_version() -> int:
 
 def hga_default_n_hi(head_dim: int, rope_base: float, span: int) -> int:
     return int(load_library().hga_default_n_hi(head_dim, rope_base, span))
+
+
+def hga_n_hi_rule(head_dim: int, rope_base: float, span: int, rule: int) -> int:
+    return int(load_library().hga_n_hi_rule(head_dim, rope_base, span, rule))
 
 
 def hga_validate(p: Params) -> int:

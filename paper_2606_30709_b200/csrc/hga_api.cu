@@ -32,7 +32,8 @@ hga_status validate(const hga_params* p) {
   if (p->io_dtype != HGA_F32 && p->io_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
   if (p->out_dtype != HGA_F32 && p->out_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
   if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05_ITEM) return HGA_ERR_INVALID_ARG;
-  if (p->reserved != 0) return HGA_ERR_INVALID_ARG;
+  if (p->rope_pos_mod < 0) return HGA_ERR_INVALID_ARG;
+  if (p->rope_pos_mod > 0 && (p->rope_pos_mod % p->chunk || p->pos0 % p->chunk)) return HGA_ERR_INVALID_ARG;
   if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
   // what the kernels implement
   if (p->chunk != kChunk) return HGA_ERR_UNSUPPORTED;
@@ -58,6 +59,7 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
   d->n_hi_c = p->n_hi_chunk >= 0 ? p->n_hi_chunk : default_n_hi(p->head_dim, p->rope_base, p->chunk);
   d->n_hi_g = p->n_hi_group >= 0 ? p->n_hi_group : default_n_hi(p->head_dim, p->rope_base, p->group);
   d->pos0 = p->pos0;
+  d->pos_mod = p->rope_pos_mod;
   d->scale = p->softmax_scale > 0.0f ? p->softmax_scale : (float)(1.0 / sqrt((double)p->head_dim));
   d->bf16_io = p->io_dtype == HGA_BF16;
   d->bf16_out = p->out_dtype == HGA_BF16;
@@ -92,6 +94,17 @@ const char* hga_status_string(hga_status s) {
 }
 
 int32_t hga_version(void) { return 100; }
+
+int32_t hga_n_hi_rule(int32_t head_dim, double rope_base, int32_t span, int32_t rule) {
+  if (head_dim <= 0 || (head_dim & 1) || !(rope_base > 0.0) || span <= 0 || rule < 0 || rule > 2) return -1;
+  if (rule == 0) return default_n_hi(head_dim, rope_base, span);
+  // theta_i * span >= c  <=>  i <= (D/2) * ln(span/c) / ln(base); evaluated pair by pair like the default rule
+  const double c = rule == 1 ? kTwoPi * 0.5 : 1.0;
+  int n = 0;
+  for (int i = 0; i < head_dim / 2; ++i)
+    if (pow(rope_base, -2.0 * (double)i / (double)head_dim) * (double)span >= c) ++n;
+  return n;
+}
 
 int32_t hga_default_n_hi(int32_t head_dim, double rope_base, int32_t span) {
   if (head_dim <= 0 || (head_dim & 1) || !(rope_base > 0.0) || span <= 0) return -1;

@@ -27,6 +27,7 @@ struct Derived {
   int F, L, L_eff, Kc, Kg;
   int n_hi_c, n_hi_g;
   long long pos0;
+  long long pos_mod;  // RoPE position wrap; 0 = off
   float scale;              // softmax scale
   bool bf16_io, bf16_out;
 };

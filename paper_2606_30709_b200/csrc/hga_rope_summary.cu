@@ -65,7 +65,7 @@ struct RsParams {
   int HK;      // heads of the "K" tensor (0: none)
   int gs, gpc, n_hi_c, n_hi_g;
   int tpr;     // tiles per row = HK + HQ
-  long long pos0;
+  long long pos0, pos_mod;
   long long total_tiles;  // rows * tpr
 };
 
@@ -174,7 +174,9 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
     if (fresh_row) {
       fresh_row = false;
       mb ^= 1;
-      const long long pos_first = p.pos0 + (long long)j * kChunk;
+      // chunk-aligned, and pos_mod is a multiple of the chunk: wrapping the chunk's first position wraps all 64
+      long long pos_first = p.pos0 + (long long)j * kChunk;
+      if (p.pos_mod > 0) pos_first %= p.pos_mod;
       const double pos = (double)(pos_first + tok);
 #pragma unroll
       for (int u = 0; u < 8; ++u) tab[u] = cos_sin_f32(pos, s_turns[i0 + u]);
@@ -370,6 +372,7 @@ RsParams base_params(const Derived& d) {
   p.PG = 1;
   p.gs = d.gs; p.gpc = d.gpc; p.n_hi_c = d.n_hi_c; p.n_hi_g = d.n_hi_g;
   p.pos0 = d.pos0;
+  p.pos_mod = d.pos_mod;
   return p;
 }
 

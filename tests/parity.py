@@ -141,7 +141,8 @@ def check_against_oracle(w: W.Workload, q, k, v, p, buf, slices, blocks, check_i
             if same_g:
                 o_out, o_lse = r.out[bi], r.lse[bi]
             else:
-                qb = oracle.round_io(oracle.rope(q[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C], op.pos0 + j * C, op.base),
+                qb = oracle.round_io(oracle.rope(q[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C], op.pos0 + j * C, op.base,
+                                                 op.pos_mod),
                                      op.io_bf16)
                 o_out, o_lse, _ = oracle.attend_block(qb, r.k_rot, kv64, int(j), C, op.gs, op.F, op.L, g_gidx[j, :max(op.Kg, 0)])
             worst["out"] = max(worst["out"], float(np.abs(g_out[:, j * C:(j + 1) * C] - o_out).max()))

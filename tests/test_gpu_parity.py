@@ -90,6 +90,40 @@ def test_small_bf16_full_parity(cfg, impl):
     parity.assert_report(rep, w, w.n_blocks * B * Hkv)
 
 
+# N3 variants: wrapped RoPE position index and the alternative high-frequency
+# thresholds -- S0..S3 feel them, S4 only through the rotated tensors and the index lists
+VARIANTS = [
+    # name, D, base, pos0, rope_pos_mod, n_hi rule
+    ("wrap_mid_sequence", 128, 1e6, 0, 1024, 0),      # positions 1024.. alias 0..
+    ("wrap_pos0_offset", 64, 1e4, 65536 - 512, 65536, 0),  # the paper's modulus, crossed at token 512
+    ("wrap_inert", 64, 1e4, 0, 65536, 0),
+    ("n_hi_half_turn", 128, 1e6, 0, 0, 1),
+    ("n_hi_one_radian_wrap", 64, 1e4, 128, 2048, 2),
+]
+
+
+@pytest.mark.parametrize("cfg", VARIANTS, ids=[c[0] for c in VARIANTS])
+def test_variants_position_wrap_and_n_hi_rules(cfg):
+    name, D, base, pos0, mod, rule = cfg
+    n_hi_c = hga.hga_n_hi_rule(D, base, 64, rule) if rule else -1
+    n_hi_g = hga.hga_n_hi_rule(D, base, 16, rule) if rule else -1
+    if rule:
+        assert (n_hi_c, n_hi_g) == (oracle.n_hi_rule(D, base, 64, rule), oracle.n_hi_rule(D, base, 16, rule))
+    w = W.Workload(name, 1, 2048, 4, 2, D, "bf16", base, topk_chunks=5, topk_groups=11, n_clusters=8, pos0=pos0,
+                   rope_pos_mod=mod, n_hi_chunk=n_hi_c, n_hi_group=n_hi_g)
+    q, k, v = W.generate(w, 13)
+    p, buf = parity.run_gpu(w, q, k, v)
+    assert p.rope_pos_mod == mod and p.n_hi_chunk == n_hi_c
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks * 2)
+    if name == "wrap_inert":  # bit-identical to the run without the modulus
+        p0, buf0 = parity.run_gpu(dataclasses.replace(w, rope_pos_mod=0), q, k, v)
+        assert torch.equal(buf.out, buf0.out) and torch.equal(buf.group_idx, buf0.group_idx)
+    if name == "wrap_mid_sequence":  # and the wrap is not a no-op
+        p0, buf0 = parity.run_gpu(dataclasses.replace(w, rope_pos_mod=0), q, k, v)
+        assert not torch.equal(buf.k_rot, buf0.k_rot)
+
+
 @pytest.mark.parametrize("impl", [ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM])
 def test_bf16_full_coverage_equals_dense(impl):
     """full chunk coverage must reproduce dense causal attention (bf16 bar: 2e-2)."""
