@@ -124,7 +124,10 @@ def check_against_oracle(w: W.Workload, q, k, v, p, buf, slices, blocks, check_i
             if n_cand and op.Kc > 0 and r.n_chunks[bi] > 0:
                 gsc = buf.chunk_score[b, kh, j].cpu().numpy()[: r.n_chunks[bi]]
                 gi = g_cidx[j, : r.n_chunks[bi]]
-                worst["score"] = max(worst["score"], float(np.abs(gsc - alls[gi]).max() / max(mx, 1e-30)))
+                # error scale of a dot product of fp32-stored operands: eps * sum_d |q_d||s_d| <= eps * |q||s|
+                # (Cauchy-Schwarz); a row whose few candidates all score near zero is not judged relative to itself
+                mag = float(np.linalg.norm(r.q_pooled[bi]) * np.linalg.norm(r.chunk_sum[gi], axis=1).max())
+                worst["score"] = max(worst["score"], float(np.abs(gsc - alls[gi]).max() / max(mx, mag, 1e-30)))
             same_g = False
             if op.Kg > 0:
                 if same_c:
