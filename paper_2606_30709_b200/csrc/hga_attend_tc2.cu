@@ -81,7 +81,7 @@ struct Smem2 {
   // barrier ids
   static constexpr int QFULL = 0, QEMPTY = 2, SFULL = 4, PFULL = 6, OFULL = 8, OEMPTY = 10, LFULL = 12, LEMPTY = 14,
                        LISTFULL = 16, LISTEMPTY = 18, KFULL = 20, KEMPTY = KFULL + kStages, VFULL = KEMPTY + kStages,
-                       VEMPTY = VFULL + kStages, kNumBars = VEMPTY + kStages;
+                       VEMPTY = VFULL + kStages, PFULLB = VEMPTY + kStages, kNumBars = PFULLB + 2;
   static constexpr int kMisc = kBar + 8 * kNumBars;  // tmem base (4 B), n_pieces[2]
   static constexpr int kInvL = kMisc + 16;           // 2 tiles x 128 rows fp32
   static constexpr int kList = kInvL + 2 * 128 * 4;  // 2 x list_cap ints
@@ -152,6 +152,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       mbar_init(BAR(L::QEMPTY + t), 1);
       mbar_init(BAR(L::SFULL + t), 1);
       mbar_init(BAR(L::PFULL + t), 4);
+      mbar_init(BAR(L::PFULLB + t), 4);
       mbar_init(BAR(L::OFULL + t), 1);
       mbar_init(BAR(L::OEMPTY + t), 4);
       mbar_init(BAR(L::LFULL + t), 4);
@@ -285,6 +286,14 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             else acc0 = add2(acc0, pack2(p0, p1));
           }
           tmem_st16(s_addr + (uint32_t)(c0 / 2), pr);  // P overlays S (already in registers)
+          if (c0 == 32) {
+            // keys 0..63 of P are in TMEM: their P V starts while the second half is still being exponentiated,
+            // which takes half a P V off the softmax -> P V -> Q K^T -> softmax latency chain of this tile
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(L::PFULL + t));
+          }
         }
         float a0, a1;
         unpack2(add2(acc0, acc1), a0, a1);
@@ -292,7 +301,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(BAR(L::PFULL + t));
+        if (lane == 0) mbar_arrive(BAR(L::PFULLB + t));
       }
       // ---- item done: hand 1/l to the epilogue warpgroup, write LSE ----------------------------------------------
       mbar_wait(BAR(L::LEMPTY + t), (n_done & 1u) ^ 1u);
@@ -497,18 +506,20 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           umma_ss_e(d, make_desc(qa + o + kLboK, kDescHi), make_desc(ka + o + kLboK, kDescHi), idesc, kk > 0 ? 1u : 0u, ld);
         }
       };
-      auto issue_pv = [&](int t, int s, int nkeys, bool first) {
+      auto issue_pv = [&](int t, int s, int kk0, int kk1, bool first) {
         const uint32_t va = ((sbase + L::kV + s * L::kTileBytes) & 0x3FFFFu) >> 4;
         const uint32_t d = tmem + (uint32_t)(256 + t * D);
         const uint32_t a = tmem + (uint32_t)(t * 128);
         // A: P_t columns [8kk, 8kk+8) (16 bf16 keys); B: V rows 16kk..16kk+15, MN-major
-        if (nkeys == kTileKeys) {
+        if (kk1 - kk0 == kPPT / 2) {
 #pragma unroll
-          for (int kk = 0; kk < kPPT; ++kk)
+          for (int u = 0; u < kPPT / 2; ++u) {
+            const int kk = kk0 + u;
             umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(va + (uint32_t)(kk * 16 * 128 >> 4) + kLboV, kDescHi), idesc_pv,
                       (!first || kk > 0) ? 1u : 0u, ld);
+          }
         } else {
-          for (int kk = 0; kk < nkeys / 16; ++kk)
+          for (int kk = kk0; kk < kk1; ++kk)
             umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(va + (uint32_t)(kk * 16 * 128 >> 4) + kLboV, kDescHi), idesc_pv,
                       (!first || kk > 0) ? 1u : 0u, ld);
         }
@@ -565,15 +576,18 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             uint32_t& oe_cnt = t == 0 ? oe_cnt0 : oe_cnt1;
             uint32_t& q_cnt = t == 0 ? q_cnt0 : q_cnt1;
             if (t < nt) {
-              mbar_wait(BAR(L::PFULL + t), p_cnt & 1u);
-              ++p_cnt;
+              mbar_wait(BAR(L::PFULL + t), p_cnt & 1u);  // keys 0..63 of P_t
               if (i == 0) {
                 // the epilogue has drained the previous item's O_t
                 mbar_wait(BAR(L::OEMPTY + t), (oe_cnt & 1u) ^ 1u);
                 ++oe_cnt;
               }
               tc_fence_after();
-              issue_pv(t, vs, nkeys, i == 0);
+              issue_pv(t, vs, 0, min(nkeys / 16, kPPT / 2), i == 0);
+              mbar_wait(BAR(L::PFULLB + t), p_cnt & 1u);  // keys 64..127
+              ++p_cnt;
+              tc_fence_after();
+              issue_pv(t, vs, kPPT / 2, nkeys / 16, false);
               if (last) umma_commit_e(BAR(L::OFULL + t), ld);
             }
             if (more && t < nt_qk) {
