@@ -32,11 +32,15 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
   return ok != 0;
 }
 // Bounded wait: a protocol bug must abort the kernel (trap -> launch failure), never hang the GPU.
+// The bound is a poll count, not a clock reading: a failed try_wait has already slept for the hardware's time limit,
+// and the poll loops of the waiting roles share issue slots with the softmax warps (ncu: 43 % of all issued
+// instructions of attend_tc2 were poll-loop instructions when every iteration read the clock).  A suspend-time hint on
+// try_wait (1 us, 20 us) was measured slower (c5 step 1.261 -> 1.273 ms): the waits are short and wake-up latency matters.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
-  const long long t0 = clock64();
+  uint32_t polls = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (clock64() - t0 > 4000000000ll) __trap();
+    if (++polls > (1u << 26)) __trap();
   }
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
