@@ -61,6 +61,7 @@ struct Tc2Params {
   int F, L_eff, gs, Kg;
   int n_mt;           // 128-row query tiles per unit = ceil(G/2)
   int ctas_per_unit;  // ceil(n_mt/2)
+  int split;          // n_mt == 1 (G <= 2): the single query tile runs on both softmax warpgroups, key tiles split even/odd
   int list_cap;       // pieces per list buffer
   int n_items;
   float scale_log2;   // softmax_scale * log2(e)
@@ -83,8 +84,8 @@ struct Smem2 {
                        LISTFULL = 16, LISTEMPTY = 18, KFULL = 20, KEMPTY = KFULL + kStages, VFULL = KEMPTY + kStages,
                        VEMPTY = VFULL + kStages, PFULLB = VEMPTY + kStages, kNumBars = PFULLB + 2;
   static constexpr int kMisc = kBar + 8 * kNumBars;  // tmem base (4 B), n_pieces[2]
-  static constexpr int kInvL = kMisc + 16;           // 2 tiles x 128 rows fp32
-  static constexpr int kList = kInvL + 2 * 128 * 4;  // 2 x list_cap ints
+  static constexpr int kInvL = kMisc + 16;           // 2 tiles x 128 rows fp32: 1/l (split mode: l), then m (split mode)
+  static constexpr int kList = kInvL + 4 * 128 * 4;  // 2 x list_cap ints
 };
 
 struct Item {
@@ -141,6 +142,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   volatile uint32_t* tmem_base_p = reinterpret_cast<volatile uint32_t*>(smem + L::kMisc);
   volatile int* s_np = reinterpret_cast<volatile int*>(smem + L::kMisc + 4);  // [2]
   float* s_invl = reinterpret_cast<float*>(smem + L::kInvL);                  // [2][128]
+  float* s_m = s_invl + 2 * 128;                                              // [2][128], split mode only
   int* s_list = reinterpret_cast<int*>(smem + L::kList);                      // [2][list_cap]
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
@@ -202,11 +204,15 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       const int n_pieces = s_np[buf];
       __syncwarp();
       if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
-      if (t >= im.nt) continue;
+      const bool split = prm.split != 0;
+      if (!split && t >= im.nt) continue;
       const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
       float m_run = -CUDART_INF_F;  // running reference max, raw logit units
       float l_run = 0.f;
-      for (int i = 0; i < n_tiles; ++i) {
+      // split mode: this warpgroup takes key tiles t, t+2, ... of the item's single query tile; the two partial
+      // (m, l, O) results are merged by the epilogue warpgroup
+      const int i_first = split ? t : 0, i_step = split ? 2 : 1;
+      for (int i = i_first; i < n_tiles; i += i_step) {
         const int nk = min(kPPT, n_pieces - i * kPPT) * 16;  // valid key columns of this tile
         mbar_wait(BAR(L::SFULL + t), s_cnt & 1u);
         ++s_cnt;
@@ -250,7 +256,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             m_run = m_new;
             l_run *= alpha;
           }
-          if (i > 0) {
+          if (i != i_first) {
             // O_t is quiescent here: S_FULL(i) was committed after PV(t, i-1)
 #pragma unroll
             for (int c0 = 0; c0 < D; c0 += 32) {
@@ -306,9 +312,10 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // ---- item done: hand 1/l to the epilogue warpgroup, write LSE ----------------------------------------------
       mbar_wait(BAR(L::LEMPTY + t), (n_done & 1u) ^ 1u);
       ++n_done;
-      s_invl[t * 128 + row] = 1.f / l_run;
+      s_invl[t * 128 + row] = split ? l_run : 1.f / l_run;
+      if (split) s_m[t * 128 + row] = m_run * sl2;  // log2 units; -inf when this half saw no key tile
       const int head_in_group = (im.mt0 + t) * 2 + row / 64;
-      if (lse != nullptr && head_in_group < prm.G) {
+      if (!split && lse != nullptr && head_in_group < prm.G) {
         const size_t orow = ((size_t)im.b * prm.Hq + (size_t)(im.kv * prm.G + head_in_group)) * prm.N + (size_t)im.j * kChunk + r64;
         lse[orow] = (m_run * sl2 + log2f(l_run)) * 0.69314718055994530942f;
       }
@@ -332,30 +339,64 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         mbar_wait(BAR(L::LFULL + t), o_cnt[t] & 1u);
         ++o_cnt[t];
         tc_fence_after();
-        const float inv = s_invl[t * 128 + e * 32 + lane];
+        float inv = s_invl[t * 128 + e * 32 + lane];
         const int head_in_group = (im.mt0 + t) * 2 + e / 2;
         const bool live = head_in_group < prm.G;
         const int grow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk + (e % 2) * 32;
         const uint32_t o_addr = tmem + lane_base + (uint32_t)(256 + t * D);
+        float w1 = 0.f;  // split mode: weight of the second partial result O_1 (0 when it saw no key tile)
+        if (prm.split) {
+          // merge the two partial softmax results of the item's single query tile (t == 0 here):
+          // m = max(m0, m1), l = l0 2^(m0-m) + l1 2^(m1-m), O = (O_0 2^(m0-m) + O_1 2^(m1-m)) / l
+          mbar_wait(BAR(L::OFULL + 1), o_cnt[1] & 1u);
+          mbar_wait(BAR(L::LFULL + 1), o_cnt[1] & 1u);
+          ++o_cnt[1];
+          tc_fence_after();
+          const int rowi = e * 32 + lane;
+          const float l0 = inv, m0 = s_m[rowi], l1 = s_invl[128 + rowi], m1 = s_m[128 + rowi];
+          const bool use1 = l1 > 0.f;
+          const float m = use1 ? fmaxf(m0, m1) : m0;  // m0 is finite: tile 0 holds the diagonal key
+          const float w0 = exp2f(m0 - m);
+          w1 = use1 ? exp2f(m1 - m) : 0.f;
+          const float l = l0 * w0 + l1 * w1;
+          inv = w0 / l;
+          w1 = w1 / l;
+          if (lse != nullptr && live) {
+            const size_t orow = ((size_t)im.b * prm.Hq + (size_t)(im.kv * prm.G + head_in_group)) * prm.N +
+                                (size_t)im.j * kChunk + (size_t)(rowi % 64);
+            lse[orow] = (m + log2f(l)) * 0.69314718055994530942f;
+          }
+        }
+        // columns [c, c + 32) of the normalised output row into dst
+        auto load_out = [&](int c, uint32_t* dst) {
+          tmem_ld32(o_addr + c, dst);
+          tmem_wait_ld();
+#pragma unroll
+          for (int u = 0; u < 32; ++u) dst[u] = __float_as_uint(__uint_as_float(dst[u]) * inv);
+          if (prm.split) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              uint32_t o1[16];
+              tmem_ld16(o_addr + D + c + 16 * h, o1);  // O_1 sits D columns after O_0
+              tmem_wait_ld();
+#pragma unroll
+              for (int u = 0; u < 16; ++u)
+                if (w1 != 0.f) dst[16 * h + u] = __float_as_uint(fmaf(__uint_as_float(o1[u]), w1, __uint_as_float(dst[16 * h + u])));
+            }
+          }
+        };
         for (int c0 = 0; c0 < D; c0 += colw) {
           uint32_t w[32];
           if (prm.out_bf16) {
             uint32_t orr[32];
-            tmem_ld32(o_addr + c0, orr);
-            tmem_wait_ld();
+            load_out(c0, orr);
 #pragma unroll
-            for (int c = 0; c < 16; ++c)
-              w[c] = cvt_bf16x2(__uint_as_float(orr[2 * c]) * inv, __uint_as_float(orr[2 * c + 1]) * inv);
-            tmem_ld32(o_addr + c0 + 32, orr);
-            tmem_wait_ld();
+            for (int c = 0; c < 16; ++c) w[c] = cvt_bf16x2(__uint_as_float(orr[2 * c]), __uint_as_float(orr[2 * c + 1]));
+            load_out(c0 + 32, orr);
 #pragma unroll
-            for (int c = 0; c < 16; ++c)
-              w[16 + c] = cvt_bf16x2(__uint_as_float(orr[2 * c]) * inv, __uint_as_float(orr[2 * c + 1]) * inv);
+            for (int c = 0; c < 16; ++c) w[16 + c] = cvt_bf16x2(__uint_as_float(orr[2 * c]), __uint_as_float(orr[2 * c + 1]));
           } else {
-            tmem_ld32(o_addr + c0, w);
-            tmem_wait_ld();
-#pragma unroll
-            for (int c = 0; c < 32; ++c) w[c] = __float_as_uint(__uint_as_float(w[c]) * inv);
+            load_out(c0, w);
           }
           if (live) {
             if (lane == 0) bulk_wait_read0();  // the previous store has finished reading the staging tile
@@ -377,6 +418,10 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         if (lane == 0) {
           mbar_arrive(BAR(L::OEMPTY + t));
           mbar_arrive(BAR(L::LEMPTY + t));
+          if (prm.split) {
+            mbar_arrive(BAR(L::OEMPTY + 1));
+            mbar_arrive(BAR(L::LEMPTY + 1));
+          }
         }
       }
     }
@@ -458,15 +503,16 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           if (active) tma_load_2d_hint(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s), pol_kv);
           if (i == 0) {
             // Q tiles of this item: (tile t, head-in-tile hh, column block cb) -> 64 rows x 64 columns
-            for (int t = 0; t < im.nt; ++t) {
+            for (int t = 0; t < (prm.split ? 2 : im.nt); ++t) {  // split mode: the same Q tile in both slots
               mbar_wait(BAR(L::QEMPTY + t), (qe_cnt[t] & 1u) ^ 1u);
               ++qe_cnt[t];
               if (lane == 0) mbar_expect_tx(BAR(L::QFULL + t), (uint32_t)L::kTileBytes);
               __syncwarp();
               if (lane < 2 * L::kHalves) {
                 const int qcb = lane % L::kHalves, hh = lane / L::kHalves;
-                int head_in_group = (im.mt0 + t) * 2 + hh;
-                if (head_in_group >= prm.G) head_in_group = (im.mt0 + t) * 2;  // odd G: duplicate a live head, never stored
+                const int tq = prm.split ? 0 : t;
+                int head_in_group = (im.mt0 + tq) * 2 + hh;
+                if (head_in_group >= prm.G) head_in_group = (im.mt0 + tq) * 2;  // odd G: duplicate a live head, never stored
                 const int qrow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk;
                 tma_load_2d_hint(sbase + L::kQ + t * L::kTileBytes + qcb * L::kHalfBytes + hh * 64 * 128, &tmQ, qcb * 64,
                                  qrow, BAR(L::QFULL + t), pol_q);
@@ -524,9 +570,77 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                       (!first || kk > 0) ? 1u : 0u, ld);
         }
       };
+      if (prm.split) {
+        // One query tile per item, two accumulators: virtual tile t (S_t, O_t, softmax warpgroup t) takes key tiles
+        // u = t, t+2, ...; each has its own softmax -> P V -> Q K^T chain, so the two chains overlap on the tensor
+        // pipe exactly like the two query tiles of the general case.  Key tile u of the item lives in stage
+        // (base + u) % kStages and is used by one virtual tile only.
+        uint32_t base = 0, q_cnt[2] = {0, 0}, p_cnt[2] = {0, 0}, oe_cnt[2] = {0, 0};
+        int k = 0;
+        for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x, ++k) {
+          const int buf = k & 1;
+          mbar_wait(BAR(L::LISTFULL + buf), (uint32_t)(k >> 1) & 1u);
+          const int n_pieces = s_np[buf];
+          const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
+          auto nkeys_of = [&](int u) { return min(kPPT, n_pieces - u * kPPT) * 16; };
+          auto st_of = [&](int u) { return (int)((base + (uint32_t)u) % L::kStages); };
+          auto ph_of = [&](int u) { return ((base + (uint32_t)u) / L::kStages) & 1u; };
+          for (int t = 0; t < 2; ++t) {  // first Q K^T of each virtual tile
+            mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+            ++q_cnt[t];
+            if (t < n_tiles) {
+              mbar_wait(BAR(L::KFULL + st_of(t)), ph_of(t));
+              tc_fence_after();
+              issue_qk(t, st_of(t), nkeys_of(t));
+              umma_commit_e(BAR(L::SFULL + t), ld);
+              umma_commit_e(BAR(L::KEMPTY + st_of(t)), ld);
+              if (t + 2 >= n_tiles) umma_commit_e(BAR(L::QEMPTY + t), ld);
+            } else if (ld) {
+              mbar_arrive(BAR(L::QEMPTY + t));  // this half has no key tile: its Q slot is free at once
+            }
+          }
+          for (int u = 0; u < n_tiles; ++u) {
+            const int t = u & 1, vs = st_of(u), nkeys = nkeys_of(u);
+            mbar_wait(BAR(L::PFULL + t), p_cnt[t] & 1u);  // keys 0..63 of P_t
+            if (u < 2) {
+              mbar_wait(BAR(L::OEMPTY + t), (oe_cnt[t] & 1u) ^ 1u);  // the epilogue has drained the previous item's O_t
+              ++oe_cnt[t];
+            }
+            mbar_wait(BAR(L::VFULL + vs), ph_of(u));
+            tc_fence_after();
+            issue_pv(t, vs, 0, min(nkeys / 16, kPPT / 2), u < 2);
+            mbar_wait(BAR(L::PFULLB + t), p_cnt[t] & 1u);  // keys 64..127
+            ++p_cnt[t];
+            tc_fence_after();
+            issue_pv(t, vs, kPPT / 2, nkeys / 16, false);
+            umma_commit_e(BAR(L::VEMPTY + vs), ld);
+            if (u + 2 < n_tiles) {
+              const int ks = st_of(u + 2);
+              mbar_wait(BAR(L::KFULL + ks), ph_of(u + 2));
+              tc_fence_after();
+              issue_qk(t, ks, nkeys_of(u + 2));
+              umma_commit_e(BAR(L::SFULL + t), ld);
+              umma_commit_e(BAR(L::KEMPTY + ks), ld);
+              if (u + 4 >= n_tiles) umma_commit_e(BAR(L::QEMPTY + t), ld);
+            } else {
+              umma_commit_e(BAR(L::OFULL + t), ld);
+            }
+          }
+          if (n_tiles < 2) {
+            // the second half saw no key tile (block 0 with a 64-key list): hand its untouched O_1 over anyway, the
+            // epilogue gives it weight 0
+            mbar_wait(BAR(L::OEMPTY + 1), (oe_cnt[1] & 1u) ^ 1u);
+            ++oe_cnt[1];
+            if (ld) mbar_arrive(BAR(L::OFULL + 1));
+          }
+          base += (uint32_t)n_tiles;
+          __syncwarp();
+          if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
+        }
+      }
       uint32_t step = 0;  // K/V tiles consumed so far: tile `step` lives in stage step % kStages
       int k = 0;
-      int it = blockIdx.x;
+      int it = prm.split ? prm.n_items : blockIdx.x;  // split mode is handled above
       int n_pieces = 0, nt = 0;
       if (it < prm.n_items) {
         mbar_wait(BAR(L::LISTFULL + 0), 0);
@@ -629,6 +743,7 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
   prm.F = d.F; prm.L_eff = d.L_eff; prm.gs = d.gs; prm.Kg = d.Kg;
   prm.n_mt = (d.G + 1) / 2;
   prm.ctas_per_unit = (prm.n_mt + 1) / 2;
+  prm.split = prm.n_mt == 1 ? 1 : 0;
   prm.list_cap = max_key_pieces(d.F, d.L_eff, d.gs, d.Kg);
   prm.scale_log2 = d.scale * 1.4426950408889634f;
   prm.out_bf16 = d.bf16_out ? 1 : 0;
