@@ -212,10 +212,22 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // split mode: this warpgroup takes key tiles t, t+2, ... of the item's single query tile; the two partial
       // (m, l, O) results are merged by the epilogue warpgroup
       const int i_first = split ? t : 0, i_step = split ? 2 : 1;
+      const bool dead = (im.mt0 + (split ? 0 : t)) * 2 + row / 64 >= prm.G;  // warp-uniform: a warp is 32 rows of one head
       for (int i = i_first; i < n_tiles; i += i_step) {
         const int nk = min(kPPT, n_pieces - i * kPPT) * 16;  // valid key columns of this tile
         mbar_wait(BAR(L::SFULL + t), s_cnt & 1u);
         ++s_cnt;
+        if (dead) {
+          // rows of a padding head (odd G, G = 1): nothing is stored from them, so no softmax either -- P stays
+          // whatever it was and only feeds O rows that are never read.  The wait above keeps the warp in step
+          // with the tile sequence (the next S arrives only after this tile's P barrier has completed).
+          __syncwarp();
+          if (lane == 0) {
+            mbar_arrive(BAR(L::PFULL + t));
+            mbar_arrive(BAR(L::PFULLB + t));
+          }
+          continue;
+        }
         tc_fence_after();
         uint32_t sr[128];
         tmem_ld32(s_addr + 0, sr + 0);
