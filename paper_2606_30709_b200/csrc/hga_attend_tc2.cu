@@ -130,7 +130,8 @@ __device__ __forceinline__ void exp2_poly2(float x0, float x1, float& p0, float&
   p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
 }
 
-template <int D>
+// kSplit: one query tile per item (G <= 2), see the MMA issuer.  kPad: some tile holds a padding head (odd G).
+template <int D, bool kSplit, bool kPad>
 __global__ void __launch_bounds__(kThreads, 1)
 attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
@@ -204,7 +205,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       const int n_pieces = s_np[buf];
       __syncwarp();
       if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
-      const bool split = prm.split != 0;
+      constexpr bool split = kSplit;
       if (!split && t >= im.nt) continue;
       const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
       float m_run = -CUDART_INF_F;  // running reference max, raw logit units
@@ -212,7 +213,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // split mode: this warpgroup takes key tiles t, t+2, ... of the item's single query tile; the two partial
       // (m, l, O) results are merged by the epilogue warpgroup
       const int i_first = split ? t : 0, i_step = split ? 2 : 1;
-      const bool dead = (im.mt0 + (split ? 0 : t)) * 2 + row / 64 >= prm.G;  // warp-uniform: a warp is 32 rows of one head
+      const bool dead = kPad && (im.mt0 + (split ? 0 : t)) * 2 + row / 64 >= prm.G;  // warp-uniform: a warp is 32 rows of one head
       for (int i = i_first; i < n_tiles; i += i_step) {
         const int nk = min(kPPT, n_pieces - i * kPPT) * 16;  // valid key columns of this tile
         mbar_wait(BAR(L::SFULL + t), s_cnt & 1u);
@@ -357,7 +358,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         const int grow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk + (e % 2) * 32;
         const uint32_t o_addr = tmem + lane_base + (uint32_t)(256 + t * D);
         float w1 = 0.f;  // split mode: weight of the second partial result O_1 (0 when it saw no key tile)
-        if (prm.split) {
+        if constexpr (kSplit) {
           // merge the two partial softmax results of the item's single query tile (t == 0 here):
           // m = max(m0, m1), l = l0 2^(m0-m) + l1 2^(m1-m), O = (O_0 2^(m0-m) + O_1 2^(m1-m)) / l
           mbar_wait(BAR(L::OFULL + 1), o_cnt[1] & 1u);
@@ -385,7 +386,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           tmem_wait_ld();
 #pragma unroll
           for (int u = 0; u < 32; ++u) dst[u] = __float_as_uint(__uint_as_float(dst[u]) * inv);
-          if (prm.split) {
+          if constexpr (kSplit) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
               uint32_t o1[16];
@@ -430,7 +431,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         if (lane == 0) {
           mbar_arrive(BAR(L::OEMPTY + t));
           mbar_arrive(BAR(L::LEMPTY + t));
-          if (prm.split) {
+          if constexpr (kSplit) {
             mbar_arrive(BAR(L::OEMPTY + 1));
             mbar_arrive(BAR(L::LEMPTY + 1));
           }
@@ -515,14 +516,14 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           if (active) tma_load_2d_hint(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s), pol_kv);
           if (i == 0) {
             // Q tiles of this item: (tile t, head-in-tile hh, column block cb) -> 64 rows x 64 columns
-            for (int t = 0; t < (prm.split ? 2 : im.nt); ++t) {  // split mode: the same Q tile in both slots
+            for (int t = 0; t < (kSplit ? 2 : im.nt); ++t) {  // split mode: the same Q tile in both slots
               mbar_wait(BAR(L::QEMPTY + t), (qe_cnt[t] & 1u) ^ 1u);
               ++qe_cnt[t];
               if (lane == 0) mbar_expect_tx(BAR(L::QFULL + t), (uint32_t)L::kTileBytes);
               __syncwarp();
               if (lane < 2 * L::kHalves) {
                 const int qcb = lane % L::kHalves, hh = lane / L::kHalves;
-                const int tq = prm.split ? 0 : t;
+                const int tq = kSplit ? 0 : t;
                 int head_in_group = (im.mt0 + tq) * 2 + hh;
                 if (head_in_group >= prm.G) head_in_group = (im.mt0 + tq) * 2;  // odd G: duplicate a live head, never stored
                 const int qrow = (im.b * prm.Hq + im.kv * prm.G + head_in_group) * prm.N + im.j * kChunk;
@@ -582,7 +583,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                       (!first || kk > 0) ? 1u : 0u, ld);
         }
       };
-      if (prm.split) {
+      if constexpr (kSplit) {
         // One query tile per item, two accumulators: virtual tile t (S_t, O_t, softmax warpgroup t) takes key tiles
         // u = t, t+2, ...; each has its own softmax -> P V -> Q K^T chain, so the two chains overlap on the tensor
         // pipe exactly like the two query tiles of the general case.  Key tile u of the item lives in stage
@@ -652,7 +653,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       }
       uint32_t step = 0;  // K/V tiles consumed so far: tile `step` lives in stage step % kStages
       int k = 0;
-      int it = prm.split ? prm.n_items : blockIdx.x;  // split mode is handled above
+      int it = kSplit ? prm.n_items : blockIdx.x;  // split mode is handled above
       int n_pieces = 0, nt = 0;
       if (it < prm.n_items) {
         mbar_wait(BAR(L::LISTFULL + 0), 0);
@@ -778,7 +779,8 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
     HGA_CUDA_OK(cudaGetDevice(&dev));
     HGA_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
   }
-  auto kern = attend_tc2_kernel<D>;
+  auto kern = prm.split ? attend_tc2_kernel<D, true, true>
+                        : (d.G % 2 ? attend_tc2_kernel<D, false, true> : attend_tc2_kernel<D, false, false>);
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int grid = (int)(n_items < n_sm ? n_items : n_sm);
   kern<<<grid, kThreads, smem, s>>>(tmQ, tmK, tmV, tmO, gi, lse, prm);
