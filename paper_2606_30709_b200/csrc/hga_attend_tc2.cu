@@ -589,28 +589,37 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         // pipe exactly like the two query tiles of the general case.  Key tile u of the item lives in stage
         // (base + u) % kStages and is used by one virtual tile only.
         uint32_t base = 0, q_cnt[2] = {0, 0}, p_cnt[2] = {0, 0}, oe_cnt[2] = {0, 0};
+        // first Q K^T of virtual tile t for an item of np pieces whose key tile 0 is global tile b0
+        auto first_qk = [&](int t, int np, uint32_t b0) {
+          const int nt_ = (np + kPPT - 1) / kPPT;
+          mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+          ++q_cnt[t];
+          if (t < nt_) {
+            const int ks = (int)((b0 + (uint32_t)t) % L::kStages);
+            mbar_wait(BAR(L::KFULL + ks), ((b0 + (uint32_t)t) / L::kStages) & 1u);
+            tc_fence_after();
+            issue_qk(t, ks, min(kPPT, np - t * kPPT) * 16);
+            umma_commit_e(BAR(L::SFULL + t), ld);
+            umma_commit_e(BAR(L::KEMPTY + ks), ld);
+            if (t + 2 >= nt_) umma_commit_e(BAR(L::QEMPTY + t), ld);
+          } else if (ld) {
+            mbar_arrive(BAR(L::QEMPTY + t));  // this half has no key tile: its Q slot is free at once
+          }
+        };
+        bool pre[2] = {false, false};  // the next item's first Q K^T of tile t went out behind this item's last P V
         int k = 0;
         for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x, ++k) {
           const int buf = k & 1;
+          const bool has_next = it + (int)gridDim.x < prm.n_items;
           mbar_wait(BAR(L::LISTFULL + buf), (uint32_t)(k >> 1) & 1u);
           const int n_pieces = s_np[buf];
           const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
           auto nkeys_of = [&](int u) { return min(kPPT, n_pieces - u * kPPT) * 16; };
           auto st_of = [&](int u) { return (int)((base + (uint32_t)u) % L::kStages); };
           auto ph_of = [&](int u) { return ((base + (uint32_t)u) / L::kStages) & 1u; };
-          for (int t = 0; t < 2; ++t) {  // first Q K^T of each virtual tile
-            mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
-            ++q_cnt[t];
-            if (t < n_tiles) {
-              mbar_wait(BAR(L::KFULL + st_of(t)), ph_of(t));
-              tc_fence_after();
-              issue_qk(t, st_of(t), nkeys_of(t));
-              umma_commit_e(BAR(L::SFULL + t), ld);
-              umma_commit_e(BAR(L::KEMPTY + st_of(t)), ld);
-              if (t + 2 >= n_tiles) umma_commit_e(BAR(L::QEMPTY + t), ld);
-            } else if (ld) {
-              mbar_arrive(BAR(L::QEMPTY + t));  // this half has no key tile: its Q slot is free at once
-            }
+          for (int t = 0; t < 2; ++t) {
+            if (!pre[t]) first_qk(t, n_pieces, base);
+            pre[t] = false;
           }
           for (int u = 0; u < n_tiles; ++u) {
             const int t = u & 1, vs = st_of(u), nkeys = nkeys_of(u);
@@ -637,6 +646,12 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
               if (u + 4 >= n_tiles) umma_commit_e(BAR(L::QEMPTY + t), ld);
             } else {
               umma_commit_e(BAR(L::OFULL + t), ld);
+              if (has_next) {
+                // S_t is free once this P V has run: queue the next item's first Q K^T of this tile right behind it
+                mbar_wait(BAR(L::LISTFULL + (buf ^ 1)), (uint32_t)((k + 1) >> 1) & 1u);
+                first_qk(t, s_np[buf ^ 1], base + (uint32_t)n_tiles);
+                pre[t] = true;
+              }
             }
           }
           if (n_tiles < 2) {
