@@ -75,6 +75,10 @@ SMALL = [
     ("d128_g2_pos0", 1, 1024, 4, 2, 128, 1e6, 4, 16, 1, 2),
     ("d64_g1_kc40", 1, 4096, 2, 2, 64, 1e4, 40, 50, 1, 1),   # K_c > 32: the generic selection kernel
     ("d64_g2_kg_lt", 1, 2048, 4, 2, 64, 1e4, 20, 33, 1, 1),  # 80 group candidates, non-trivial top-33
+    # split mode of the persistent S4 kernel (G <= 2): even / odd key-tile counts, a 64-key partial tail, two stages
+    ("d64_g1_two_tiles", 1, 1024, 2, 2, 64, 1e4, 2, 4, 1, 1),     # 256 keys = 2 tiles
+    ("d128_g1_three_tiles", 1, 1024, 2, 2, 128, 1e6, 2, 8, 1, 1),  # 320 keys = 2.5 tiles, D 128 (two K/V stages)
+    ("d64_g2_five_tiles", 1, 2048, 4, 2, 64, 1e4, 8, 28, 0, 1),   # 576 keys = 4.5 tiles, no sink
 ]
 
 
@@ -171,8 +175,9 @@ def test_attend_isolated_caller_supplied_lists(impl):
             assert np.abs(lse[0, kh * G:(kh + 1) * G, j * C:(j + 1) * C] - rl).max() <= 2e-2
 
 
-def test_bf16_output_dtype():
-    w = W.Workload("bf16out", 1, 512, 4, 2, 64, "bf16", 1e4, topk_chunks=2, topk_groups=4, n_clusters=4)
+@pytest.mark.parametrize("heads", [(4, 2), (8, 1), (3, 1), (2, 2)], ids=["g2", "g8", "g3", "g1"])
+def test_bf16_output_dtype(heads):
+    w = W.Workload("bf16out", 1, 512, heads[0], heads[1], 64, "bf16", 1e4, topk_chunks=2, topk_groups=4, n_clusters=4)
     q, k, v = W.generate(w, 2)
     p, buf = parity.run_gpu(w, q, k, v, out_dtype=HGA_F32)
     p2, buf2 = parity.run_gpu(w, q, k, v, out_dtype=HGA_BF16)
