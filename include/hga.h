@@ -237,7 +237,9 @@ HGA_API hga_status hga_prefill_profile(const hga_params* p, const hga_buffers* b
  * Host-buffer path.  A plan owns every device buffer of one prefill pass for `p` plus a private stream.
  * hga_host_prefill copies q/k/v from HOST memory (pinned for full speed; pageable works), runs S0..S4, copies `out`
  * (and, if non-null, group_idx [batch,n_kv_heads,seq/chunk,topk_groups] and lse) back to HOST memory and returns
- * after the stream has drained.  *_host buffers have the layouts above.
+ * after the stream has drained.  *_host buffers have the layouts above.  The work is pipelined over independent
+ * (batch, KV head) parts on three streams, and for long sequences every part is cut into runs of whole chunks
+ * (hga_prefill_window steps), so copies in, kernels and copies out overlap; results are bit-identical to hga_prefill.
  */
 typedef struct hga_host_plan hga_host_plan;
 HGA_API hga_status hga_host_plan_create(const hga_params* p, hga_host_plan** plan);

@@ -279,6 +279,9 @@ struct hga_host_plan {
   // the work is pipelined over parts: runs of kv_per_part KV heads of one batch item (batch_per_part == 1), or
   // batch_per_part whole batch items (kv_per_part == n_kv_heads)
   int n_parts, kv_per_part, batch_per_part;
+  // every part is further cut into n_seq runs of whole chunks (hga_prefill_window steps), so that the first kernels
+  // start after 1/n_seq of a part has arrived and the first results leave after 1/n_seq of its attention
+  int n_seq;
   void* arena;
   size_t arena_bytes;
   hga_buffers buf;
@@ -339,11 +342,14 @@ hga_status hga_host_plan_create(const hga_params* p, hga_host_plan** out_plan) {
       if (d.Hkv % m == 0 && d.B * (d.Hkv / m) >= 4) { pl->kv_per_part = m; break; }
   }
   pl->n_parts = (d.B / pl->batch_per_part) * (d.Hkv / pl->kv_per_part);
-  pl->ev_in = new (std::nothrow) cudaEvent_t[pl->n_parts]();
-  pl->ev_done = new (std::nothrow) cudaEvent_t[pl->n_parts]();
+  pl->n_seq = 1;
+  while (pl->n_seq < 8 && d.n_b % (2 * pl->n_seq) == 0 && d.N / (2 * pl->n_seq) >= 8192) pl->n_seq *= 2;
+  const int n_ev = pl->n_parts * pl->n_seq;
+  pl->ev_in = new (std::nothrow) cudaEvent_t[n_ev]();
+  pl->ev_done = new (std::nothrow) cudaEvent_t[n_ev]();
   bool ok = pl->ev_in && pl->ev_done && cudaStreamCreateWithFlags(&pl->s_in, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&pl->s_out, cudaStreamNonBlocking) == cudaSuccess;
-  for (int i = 0; ok && i < pl->n_parts; ++i)
+  for (int i = 0; ok && i < n_ev; ++i)
     ok = cudaEventCreateWithFlags(&pl->ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&pl->ev_done[i], cudaEventDisableTiming) == cudaSuccess;
   if (!ok) { cudaFree(pl->arena); delete[] pl->ev_in; delete[] pl->ev_done; delete pl; return HGA_ERR_CUDA; }
@@ -379,11 +385,6 @@ hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k
   for (int i = 0; i < pl->n_parts; ++i) {
     // parts tile every tensor contiguously: element offsets are i * part size
     const size_t qo = (size_t)i * q_part, ko = (size_t)i * kv_part, uo = (size_t)i * unit_part;
-    HGA_CUDA_OK(cudaMemcpyAsync(off(pl->buf.k_raw, ko * e), off(k_host, ko * e), kv_part * e, cudaMemcpyHostToDevice, pl->s_in));
-    HGA_CUDA_OK(cudaMemcpyAsync(off(pl->buf.q_raw, qo * e), off(q_host, qo * e), q_part * e, cudaMemcpyHostToDevice, pl->s_in));
-    HGA_CUDA_OK(cudaMemcpyAsync(off(pl->buf.v, ko * e), off(v_host, ko * e), kv_part * e, cudaMemcpyHostToDevice, pl->s_in));
-    HGA_CUDA_OK(cudaEventRecord(pl->ev_in[i], pl->s_in));
-    HGA_CUDA_OK(cudaStreamWaitEvent(pl->stream, pl->ev_in[i], 0));
     hga_buffers b = pl->buf;
     b.q_raw = off(pl->buf.q_raw, qo * e); b.q_rot = off(pl->buf.q_rot, qo * e);
     b.k_raw = off(pl->buf.k_raw, ko * e); b.k_rot = off(pl->buf.k_rot, ko * e);
@@ -394,17 +395,37 @@ hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k
     b.group_idx = pl->buf.group_idx + uo * (d.Kg > 0 ? d.Kg : 1);
     b.out = off(pl->buf.out, qo * eo);
     b.lse = lse_host ? pl->buf.lse + (size_t)i * lse_part : nullptr;
-    // the score workspace is shared: parts run one after another on the compute stream
-    hga_status st = hga_prefill(&sp, &b, (void*)pl->stream);
-    if (st != HGA_OK) return st;
-    HGA_CUDA_OK(cudaEventRecord(pl->ev_done[i], pl->stream));
-    HGA_CUDA_OK(cudaStreamWaitEvent(pl->s_out, pl->ev_done[i], 0));
-    HGA_CUDA_OK(cudaMemcpyAsync(off(out_host, qo * eo), b.out, q_part * eo, cudaMemcpyDeviceToHost, pl->s_out));
-    if (group_idx_host && d.Kg > 0)
-      HGA_CUDA_OK(cudaMemcpyAsync(group_idx_host + uo * d.Kg, b.group_idx, unit_part * d.Kg * 4, cudaMemcpyDeviceToHost,
-                                  pl->s_out));
-    if (lse_host)
-      HGA_CUDA_OK(cudaMemcpyAsync(lse_host + (size_t)i * lse_part, b.lse, lse_part * 4, cudaMemcpyDeviceToHost, pl->s_out));
+    // the score workspace is shared: parts (and their runs) go one after another on the compute stream
+    const int heads_q = nb * m * d.G, heads_kv = nb * m;
+    const size_t row_in = (size_t)d.N * d.D * e, row_out = (size_t)d.N * d.D * eo;  // one head of Q/K/V, of out
+    for (int c = 0; c < pl->n_seq; ++c) {
+      const int ie = i * pl->n_seq + c;
+      const int j0 = d.n_b / pl->n_seq * c, j1 = d.n_b / pl->n_seq * (c + 1);  // blocks of this run
+      const size_t t0 = (size_t)j0 * d.C, nt = (size_t)(j1 - j0) * d.C;         // its tokens
+      // rows [t0, t0 + nt) of every head: one strided copy per tensor
+      HGA_CUDA_OK(cudaMemcpy2DAsync(off(b.k_raw, t0 * d.D * e), row_in, off(k_host, (ko + t0 * d.D) * e), row_in, nt * d.D * e,
+                                    heads_kv, cudaMemcpyHostToDevice, pl->s_in));
+      HGA_CUDA_OK(cudaMemcpy2DAsync(off(b.q_raw, t0 * d.D * e), row_in, off(q_host, (qo + t0 * d.D) * e), row_in, nt * d.D * e,
+                                    heads_q, cudaMemcpyHostToDevice, pl->s_in));
+      HGA_CUDA_OK(cudaMemcpy2DAsync(off(b.v, t0 * d.D * e), row_in, off(v_host, (ko + t0 * d.D) * e), row_in, nt * d.D * e,
+                                    heads_kv, cudaMemcpyHostToDevice, pl->s_in));
+      HGA_CUDA_OK(cudaEventRecord(pl->ev_in[ie], pl->s_in));
+      HGA_CUDA_OK(cudaStreamWaitEvent(pl->stream, pl->ev_in[ie], 0));
+      hga_status st = pl->n_seq == 1 ? hga_prefill(&sp, &b, (void*)pl->stream)
+                                     : hga_prefill_window(&sp, &b, (int64_t)t0, (int64_t)(t0 + nt), (void*)pl->stream);
+      if (st != HGA_OK) return st;
+      HGA_CUDA_OK(cudaEventRecord(pl->ev_done[ie], pl->stream));
+      HGA_CUDA_OK(cudaStreamWaitEvent(pl->s_out, pl->ev_done[ie], 0));
+      HGA_CUDA_OK(cudaMemcpy2DAsync(off(out_host, (qo + t0 * d.D) * eo), row_out, off(b.out, t0 * d.D * eo), row_out,
+                                    nt * d.D * eo, heads_q, cudaMemcpyDeviceToHost, pl->s_out));
+      if (group_idx_host && d.Kg > 0)
+        HGA_CUDA_OK(cudaMemcpy2DAsync(group_idx_host + (uo + j0) * d.Kg, (size_t)d.n_b * d.Kg * 4, b.group_idx + (size_t)j0 * d.Kg,
+                                      (size_t)d.n_b * d.Kg * 4, (size_t)(j1 - j0) * d.Kg * 4, heads_kv, cudaMemcpyDeviceToHost,
+                                      pl->s_out));
+      if (lse_host)
+        HGA_CUDA_OK(cudaMemcpy2DAsync(lse_host + (size_t)i * lse_part + t0, (size_t)d.N * 4, b.lse + t0, (size_t)d.N * 4, nt * 4,
+                                      heads_q, cudaMemcpyDeviceToHost, pl->s_out));
+    }
   }
   HGA_CUDA_OK(cudaStreamSynchronize(pl->s_out));
   HGA_CUDA_OK(cudaStreamSynchronize(pl->stream));
@@ -413,7 +434,7 @@ hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k
 
 void hga_host_plan_destroy(hga_host_plan* pl) {
   if (!pl) return;
-  for (int i = 0; i < pl->n_parts; ++i) {
+  for (int i = 0; i < pl->n_parts * pl->n_seq; ++i) {
     cudaEventDestroy(pl->ev_in[i]);
     cudaEventDestroy(pl->ev_done[i]);
   }

@@ -184,3 +184,30 @@ def test_paper_needle_parameters_ragged_64k_p5():
         for j in (0, 3, 10, 11, 12, 31, 500 + kh, 1023):
             _check_step(_One, op, qs, ks, vs, view, j * 64, (j + 1) * 64, parity.TOL_OUT["bf16"])
         _check_step(_One, op, qs, ks, vs, view, 1024 * 64, w.n_tokens, parity.TOL_OUT["bf16"])  # ragged tail block
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# host-buffer path: hga_host_prefill pipelines H2D / S0..S4 / D2H over (batch, KV head) parts and, for long
+# sequences, over runs of chunks (hga_prefill_window steps); it must return exactly what the device path returns
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(1, 32768, 4, 2, 64), (2, 2048, 6, 2, 128), (4, 1024, 2, 2, 64)],
+                         ids=["n32k_two_runs", "b2_g3", "b4_g1"])
+def test_host_prefill_equals_device_path(shape):
+    B, N, Hq, Hkv, D = shape
+    w = W.Workload("host", B, N, Hq, Hkv, D, "bf16", 1e4 if D == 64 else 1e6, topk_chunks=6, topk_groups=20, n_clusters=8)
+    q, k, v = W.generate(w, 21)
+    p, buf = parity.run_gpu(w, q, k, v)
+    to_host = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(torch.bfloat16).pin_memory()
+    hq, hk, hv = to_host(q), to_host(k), to_host(v)
+    out = torch.full((B, Hq, N, D), float("nan"), dtype=torch.float32).pin_memory()
+    gidx = torch.full((B, Hkv, N // 64, 20), -7, dtype=torch.int32).pin_memory()
+    lse = torch.full((B, Hq, N), float("nan"), dtype=torch.float32).pin_memory()
+    plan = hga.HostPlan(p)
+    try:
+        for _ in range(2):  # a plan is reusable
+            plan.prefill(hq, hk, hv, out, gidx, lse)
+            assert torch.equal(out, buf.out.cpu())
+            assert torch.equal(gidx, buf.group_idx.cpu())
+            assert torch.equal(lse, buf.lse.cpu())
+    finally:
+        plan.close()
