@@ -191,7 +191,7 @@ def test_paper_needle_parameters_ragged_64k_p5():
 # sequences, over runs of chunks (hga_prefill_window steps); it must return exactly what the device path returns
 # ---------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("shape", [(1, 32768, 4, 2, 64), (2, 2048, 6, 2, 128), (4, 1024, 2, 2, 64)],
-                         ids=["n32k_two_runs", "b2_g3", "b4_g1"])
+                         ids=["n32k_chunk_runs", "b2_g3", "b4_g1"])
 def test_host_prefill_equals_device_path(shape):
     B, N, Hq, Hkv, D = shape
     w = W.Workload("host", B, N, Hq, Hkv, D, "bf16", 1e4 if D == 64 else 1e6, topk_chunks=6, topk_groups=20, n_clusters=8)
