@@ -12,6 +12,14 @@
 //   warp 13          TMA producer: gathers the K and V pieces of the key list (16 rows x 64 bf16 boxes, 128B swizzle)
 //   warp 14          key-list builder for the next item (double buffered)
 //
+// P_t is handed to the tensor pipe in two halves (keys 0..63 while 64..127 are still being exponentiated), which takes
+// half a P V off the tile's softmax -> P V -> Q K^T latency chain.
+//
+// Split mode (template kSplit; G <= 2, i.e. one query tile per item): the tile runs on BOTH softmax warpgroups --
+// virtual tile t owns (S_t, O_t) and the key tiles t, t+2, ... -- so two chains overlap on the tensor pipe as in the
+// general case; the epilogue merges the two partial (m, l, O) results.  kPad (odd G, G = 1): softmax warps whose 32
+// rows belong to the padding head skip the arithmetic and only keep the barrier sequence.
+//
 // Key order inside an item: current chunk first (so the causal mask lives only in columns 0..63 of tile 0), then
 // sink chunks, routed groups, local chunks; only the last 128-key tile can be partial.
 // TMEM map (512 columns): S_t at t*128 (P_t overlays its first 64 columns), O_t at 256 + t*D.
