@@ -346,6 +346,25 @@ def run_ours(args, w):
     same = bool(torch.equal(out_host.cuda(), buf.out))
     plan.close()
 
+    # ---- N1 streaming steps at the end of the context (hga_prefill_window on the filled cache): the last 64-token
+    #      chunk as one prefill step, and one single-token decode step.  Idempotent: they rewrite what is there.
+    def time_window(t_begin, t_end, reps=20):
+        for _ in range(3):
+            hga.hga_prefill_window(p, dq, dk, dv, buf, t_begin, t_end)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            hga.hga_prefill_window(p, dq, dk, dv, buf, t_begin, t_end)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    streaming = {"context": w.seq, "chunk_step_ms": time_window(w.seq - w.chunk, w.seq),
+                 "decode_step_ms": time_window(w.seq - 1, w.seq),
+                 "what": "hga_prefill_window over the last chunk [N-64, N) and over the last token [N-1, N) of the "
+                         "filled cache, all batch items and heads; CUDA events, mean of 20 calls (launch-bound)"}
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -418,6 +437,7 @@ def run_ours(args, w):
         "roofline": roof,
         "cpu_baseline": cpu,
         "stages": stages,
+        "streaming": streaming,
         "roofline_floor_ms": roofline_floor_ms,
         "frac_of_roofline_floor": roofline_floor_ms / ms_per_step,
     }

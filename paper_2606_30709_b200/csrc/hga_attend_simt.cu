@@ -55,6 +55,10 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
     l_s[threadIdx.x] = 0.f;
   }
   const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+  // rows of this block inside the token window (a streaming step may cover one token): threads and warps whose rows are
+  // all outside it skip the arithmetic -- a decode step then costs the gathers plus one live row, not a 64-row tile
+  const int r_lo = max(0, tw0 - j * 64), r_hi = min(64, tw1 - j * 64);
+  const bool thread_live = ty * 4 < r_hi && ty * 4 + 4 > r_lo;
   constexpr int OC = D / 16;  // output columns per thread
   float o[4][OC];
 #pragma unroll
@@ -88,7 +92,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
       for (int a = 0; a < 4; ++a)
 #pragma unroll
         for (int c = 0; c < 4; ++c) acc[a][c] = 0.f;
-      for (int d0 = 0; d0 < D; d0 += 4) {
+      for (int d0 = 0; thread_live && d0 < D; d0 += 4) {
         float4 qa[4], kb[4];
 #pragma unroll
         for (int a = 0; a < 4; ++a) qa[a] = *reinterpret_cast<const float4*>(Qs + (ty * 4 + a) * KP + d0);
@@ -111,7 +115,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
           const int row = ty * 4 + a, col = tx + 16 * c;
           float sv = acc[a][c] * scale;
           // validity: inside the tile, and causal (key position <= query position, Eq. 1)
-          bool ok = col < np * 16;
+          bool ok = col < np * 16 && row >= r_lo && row < r_hi;
           if (ok) {
             int key_pos = list[p0 + col / 16] * 16 + (col % 16);
             ok = key_pos <= j * 64 + row;
@@ -123,6 +127,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
     // online softmax: warp w owns rows 8w..8w+7
     for (int rr = 0; rr < 8; ++rr) {
       const int row = warp * 8 + rr;
+      if (row < r_lo || row >= r_hi) continue;  // warp-uniform
       float s0 = Ss[row * 65 + lane], s1 = Ss[row * 65 + lane + 32];
       float mx = fmaxf(s0, s1);
 #pragma unroll
@@ -154,7 +159,7 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
 #pragma unroll
         for (int c = 0; c < OC; ++c) o[a][c] *= al[a];
       const int nk = np * 16;
-      for (int kk = 0; kk < nk; ++kk) {
+      for (int kk = 0; thread_live && kk < nk; ++kk) {
         float pv[4], vv[OC];
 #pragma unroll
         for (int a = 0; a < 4; ++a) pv[a] = Ss[(ty * 4 + a) * 65 + kk];
