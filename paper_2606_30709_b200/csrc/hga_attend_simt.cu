@@ -192,10 +192,108 @@ __global__ void __launch_bounds__(kT) attend_simt_kernel(const T* __restrict__ q
     lse[((size_t)b * Hq + h) * N + (size_t)j * 64 + threadIdx.x] = m_s[threadIdx.x] + logf(l_s[threadIdx.x]);
 }
 
+// A few query rows of one block (single-token decode, a short append): one CTA per (batch, query head), the key
+// list split over 8 warps that each run an online softmax over their keys (a lane holds D/32 dimensions of q, o and
+// of every key / value row; one warp-wide dot product per key), then the 8 partial (m, l, o) results are merged.
+// Same arithmetic as the tile kernel above (fp32, exact causal rule), without its 64-row tile.
+template <typename T, typename TO, int D>
+__global__ void __launch_bounds__(256) attend_rows_kernel(const T* __restrict__ q, const T* __restrict__ k,
+                                                          const T* __restrict__ v, const int32_t* __restrict__ group_idx,
+                                                          TO* __restrict__ out, float* __restrict__ lse, int Hq, int Hkv, int N,
+                                                          int n_b, int F, int L_eff, int gs, int Kg, float scale, int list_cap,
+                                                          int j, int tw0, int tw1) {
+  constexpr int DL = D / 32, NWARP = 8;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float* part = reinterpret_cast<float*>(smem_raw);      // [NWARP][D + 2]: o, m, l
+  int* list = reinterpret_cast<int*>(part + NWARP * (D + 2));  // [list_cap] 16-token pieces
+  __shared__ int s_count;
+  const int h = blockIdx.x, b = blockIdx.y;
+  const int G = Hq / Hkv, kv = h / G;
+  const int32_t* gi = group_idx ? group_idx + (((size_t)b * Hkv + kv) * n_b + j) * Kg : nullptr;
+  const int n_keys = build_key_list(list, &s_count, j, F, L_eff, gs, Kg, gi) * 16;
+  const T* kbase = k + ((size_t)b * Hkv + kv) * (size_t)N * D;
+  const T* vbase = v + ((size_t)b * Hkv + kv) * (size_t)N * D;
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const int r_lo = max(0, tw0 - j * 64), r_hi = min(64, tw1 - j * 64);
+  for (int r = r_lo; r < r_hi; ++r) {
+    const int t_abs = j * 64 + r;
+    const T* qrow = q + (((size_t)b * Hq + h) * N + (size_t)t_abs) * D + lane * DL;
+    float qv[DL], o[DL];
+#pragma unroll
+    for (int u = 0; u < DL; ++u) {
+      qv[u] = ld_as_float(qrow + u) * scale;
+      o[u] = 0.f;
+    }
+    float m = -CUDART_INF_F, l = 0.f;
+    for (int kidx = warp; kidx < n_keys; kidx += NWARP) {
+      const int tok = list[kidx / 16] * 16 + (kidx % 16);
+      if (tok > t_abs || tok >= tw1) continue;  // causal (Eq. 1); warp-uniform
+      const T* krow = kbase + (size_t)tok * D + lane * DL;
+      const T* vrow = vbase + (size_t)tok * D + lane * DL;
+      float sdot = 0.f, vv[DL];
+#pragma unroll
+      for (int u = 0; u < DL; ++u) {
+        sdot = fmaf(qv[u], ld_as_float(krow + u), sdot);
+        vv[u] = ld_as_float(vrow + u);
+      }
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) sdot += __shfl_xor_sync(0xffffffffu, sdot, off);
+      const float m_new = fmaxf(m, sdot);
+      const float alpha = expf(m - m_new), pw = expf(sdot - m_new);  // exp(-inf) = 0 on the first key
+      l = l * alpha + pw;
+#pragma unroll
+      for (int u = 0; u < DL; ++u) o[u] = fmaf(pw, vv[u], o[u] * alpha);
+      m = m_new;
+    }
+    float* pr = part + warp * (D + 2);
+#pragma unroll
+    for (int u = 0; u < DL; ++u) pr[lane * DL + u] = o[u];
+    if (lane == 0) {
+      pr[D] = m;
+      pr[D + 1] = l;
+    }
+    __syncthreads();
+    if (warp == 0) {
+      float M = -CUDART_INF_F;
+#pragma unroll
+      for (int w = 0; w < NWARP; ++w) M = fmaxf(M, part[w * (D + 2) + D]);  // finite: the row's own key is always there
+      float L = 0.f, acc[DL];
+#pragma unroll
+      for (int u = 0; u < DL; ++u) acc[u] = 0.f;
+#pragma unroll
+      for (int w = 0; w < NWARP; ++w) {
+        const float wgt = expf(part[w * (D + 2) + D] - M);  // 0 for a warp that saw no key
+        L = fmaf(part[w * (D + 2) + D + 1], wgt, L);
+#pragma unroll
+        for (int u = 0; u < DL; ++u) acc[u] = fmaf(part[w * (D + 2) + lane * DL + u], wgt, acc[u]);
+      }
+      TO* orow = out + (((size_t)b * Hq + h) * N + (size_t)t_abs) * D + lane * DL;
+      const float inv = 1.f / L;
+#pragma unroll
+      for (int u = 0; u < DL; ++u) {
+        if constexpr (sizeof(TO) == 4) orow[u] = acc[u] * inv;
+        else orow[u] = __float2bfloat16_rn(acc[u] * inv);
+      }
+      if (lse != nullptr && lane == 0) lse[((size_t)b * Hq + h) * N + (size_t)t_abs] = M + logf(L);
+    }
+    __syncthreads();
+  }
+}
+
 template <typename T, typename TO, int D>
 hga_status launch_t(const Derived& d, const void* q, const void* k, const void* v, const int32_t* gi, void* out, float* lse,
                     cudaStream_t s) {
   const int list_cap = max_key_pieces(d.F, d.L_eff, d.gs, d.Kg);
+  const long long live_rows = d.tw1 - (d.tw0 > (long long)d.jb * 64 ? d.tw0 : (long long)d.jb * 64);
+  if (d.nj == 1 && live_rows <= 4) {  // decode / short append: no 64-row tile
+    const size_t smem_r = sizeof(float) * 8 * (D + 2) + sizeof(int) * (size_t)list_cap;
+    if (smem_r > 200 * 1024) return HGA_ERR_UNSUPPORTED;
+    auto kern_r = attend_rows_kernel<T, TO, D>;
+    HGA_CUDA_OK(cudaFuncSetAttribute(kern_r, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_r));
+    kern_r<<<dim3(d.Hq, d.B), 256, smem_r, s>>>((const T*)q, (const T*)k, (const T*)v, gi, (TO*)out, lse, d.Hq, d.Hkv, d.N, d.n_b,
+                                                d.F, d.L_eff, d.gs, d.Kg, d.scale, list_cap, d.jb, (int)d.tw0, (int)d.tw1);
+    return launch_status();
+  }
   const size_t smem = sizeof(float) * (2 * 64 * (D + 4) + 64 * D + 64 * 65 + 3 * 64) + sizeof(int) * (size_t)list_cap;
   if (smem > 220 * 1024) return HGA_ERR_UNSUPPORTED;
   auto kern = attend_simt_kernel<T, TO, D>;

@@ -119,13 +119,19 @@ def test_ragged_prefill_then_decode_matches_oracle_step(w, impl):
     hga.hga_prefill_window(p, *live, buf, 960, 961)
     torch.cuda.synchronize()
     _check_step(w, op, q, k, v, buf, 960, 961, tol)
+    # short appends: up to 4 rows go through the few-rows attention kernel (like a decode step), 5 through the tile one
+    for (a, b) in ((961, 964), (964, 968), (968, 973)):
+        _feed(live, full, a, b)
+        hga.hga_prefill_window(p, *live, buf, a, b)
+        torch.cuda.synchronize()
+        _check_step(w, op, q, k, v, buf, a, b, tol)
     # the summaries written by the streaming steps equal a vectorised pass over the closed chunks
     ref = hga.hga_prefill(p, *full)
     torch.cuda.synchronize()
     assert torch.equal(buf.chunk_sum[:, :, :15], ref.chunk_sum[:, :, :15])
     assert torch.equal(buf.group_sum[:, :, :60], ref.group_sum[:, :, :60])
-    assert torch.equal(buf.k_rot[:, :, :961], ref.k_rot[:, :, :961])
-    assert bool(torch.isnan(buf.k_rot[:, :, 961:].float()).all())  # nothing past the last step was written
+    assert torch.equal(buf.k_rot[:, :, :973], ref.k_rot[:, :, :973])
+    assert bool(torch.isnan(buf.k_rot[:, :, 973:].float()).all())  # nothing past the last step was written
 
 
 def test_window_argument_errors():
