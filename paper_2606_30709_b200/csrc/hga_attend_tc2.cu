@@ -60,6 +60,10 @@ constexpr int kRegsSoftmax = 200, kRegsEpi = 64, kRegsCtl = 48;  // 2*128*200 + 
 #ifndef HGA_S4_EMU_COUNT
 #define HGA_S4_EMU_COUNT 0  // measured at c5 (S4 ms): 0/4 -> 0.987, 1/8 -> 1.033, 1/4 -> 1.063, 3/8 -> 1.097, 1/2 -> 1.144
 #endif
+#ifndef HGA_S4_DIAG
+#define HGA_S4_DIAG 0  // experiments only, bit mask: 1 = no softmax arithmetic, 2 = no MMAs, 4 = no MUFU, 8 = no K/V TMA
+#endif
+constexpr int kDiag = HGA_S4_DIAG;
 constexpr int kEmuPeriod = HGA_S4_EMU_PERIOD;
 constexpr int kEmuCount = HGA_S4_EMU_COUNT;
 
@@ -221,7 +225,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // split mode: this warpgroup takes key tiles t, t+2, ... of the item's single query tile; the two partial
       // (m, l, O) results are merged by the epilogue warpgroup
       const int i_first = split ? t : 0, i_step = split ? 2 : 1;
-      const bool dead = kPad && (im.mt0 + (split ? 0 : t)) * 2 + row / 64 >= prm.G;  // warp-uniform: a warp is 32 rows of one head
+      const bool dead = (kDiag & 1) || kPad && (im.mt0 + (split ? 0 : t)) * 2 + row / 64 >= prm.G;  // warp-uniform: a warp is 32 rows of one head
       for (int i = i_first; i < n_tiles; i += i_step) {
         const int nk = min(kPPT, n_pieces - i * kPPT) * 16;  // valid key columns of this tile
         mbar_wait(BAR(L::SFULL + t), s_cnt & 1u);
@@ -305,8 +309,8 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             if ((pi % kEmuPeriod) < kEmuCount) {
               exp2_poly2(x0, x1, p0, p1);
             } else {
-              p0 = fast_exp2(x0);
-              p1 = fast_exp2(x1);
+              p0 = (kDiag & 4) ? x0 * x0 : fast_exp2(x0);
+              p1 = (kDiag & 4) ? x1 * x1 : fast_exp2(x1);
             }
             pr[c] = cvt_bf16x2(p0, p1);  // low half = key 2c, high half = key 2c+1
             if (c & 1) acc1 = add2(acc1, pack2(p0, p1));
@@ -519,9 +523,13 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           const int row = active ? kv_row0 + list[i * kPPT + pc] * 16 : 0;
           const uint32_t off = (uint32_t)(s * L::kTileBytes + cb * L::kHalfBytes + pc * 16 * 128);
           mbar_wait(BAR(L::KEMPTY + s), ph ^ 1u);
-          if (lane == 0) mbar_expect_tx(BAR(L::KFULL + s), bytes);
-          __syncwarp();
-          if (active) tma_load_2d_hint(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s), pol_kv);
+          if (kDiag & 8) {
+            if (lane == 0) mbar_arrive(BAR(L::KFULL + s));
+          } else {
+            if (lane == 0) mbar_expect_tx(BAR(L::KFULL + s), bytes);
+            __syncwarp();
+            if (active) tma_load_2d_hint(sbase + L::kK + off, &tmK, cb * 64, row, BAR(L::KFULL + s), pol_kv);
+          }
           if (i == 0) {
             // Q tiles of this item: (tile t, head-in-tile hh, column block cb) -> 64 rows x 64 columns
             for (int t = 0; t < (kSplit ? 2 : im.nt); ++t) {  // split mode: the same Q tile in both slots
@@ -541,9 +549,13 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             }
           }
           mbar_wait(BAR(L::VEMPTY + s), ph ^ 1u);
-          if (lane == 0) mbar_expect_tx(BAR(L::VFULL + s), bytes);
-          __syncwarp();
-          if (active) tma_load_2d_hint(sbase + L::kV + off, &tmV, cb * 64, row, BAR(L::VFULL + s), pol_kv);
+          if (kDiag & 8) {
+            if (lane == 0) mbar_arrive(BAR(L::VFULL + s));
+          } else {
+            if (lane == 0) mbar_expect_tx(BAR(L::VFULL + s), bytes);
+            __syncwarp();
+            if (active) tma_load_2d_hint(sbase + L::kV + off, &tmV, cb * 64, row, BAR(L::VFULL + s), pol_kv);
+          }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
@@ -553,6 +565,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // The whole warp runs the control flow convergently (so operands stay warp-uniform and ptxas needs no
       // per-lane broadcast loops); only the tcgen05 instructions themselves are predicated on one elected lane.
       const uint32_t ld = elect_one();
+      const uint32_t ldm = (kDiag & 2) ? 0u : ld;  // MMA issue predicate
       const uint32_t idesc_pv = umma_idesc(128, D, /*b_mn_major=*/true);
       const uint32_t idesc_qk_full = umma_idesc(128, kTileKeys, false);
       // descriptor high words are constant: SBO = 1024 B, version 1, SWIZZLE_128B
@@ -570,7 +583,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t o = (uint32_t)((kk / 4) * L::kHalfBytes + (kk % 4) * 32) >> 4;
-          umma_ss_e(d, make_desc(qa + o + kLboK, kDescHi), make_desc(ka + o + kLboK, kDescHi), idesc, kk > 0 ? 1u : 0u, ld);
+          umma_ss_e(d, make_desc(qa + o + kLboK, kDescHi), make_desc(ka + o + kLboK, kDescHi), idesc, kk > 0 ? 1u : 0u, ldm);
         }
       };
       auto issue_pv = [&](int t, int s, int kk0, int kk1, bool first) {
@@ -583,12 +596,12 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           for (int u = 0; u < kPPT / 2; ++u) {
             const int kk = kk0 + u;
             umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(va + (uint32_t)(kk * 16 * 128 >> 4) + kLboV, kDescHi), idesc_pv,
-                      (!first || kk > 0) ? 1u : 0u, ld);
+                      (!first || kk > 0) ? 1u : 0u, ldm);
           }
         } else {
           for (int kk = kk0; kk < kk1; ++kk)
             umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(va + (uint32_t)(kk * 16 * 128 >> 4) + kLboV, kDescHi), idesc_pv,
-                      (!first || kk > 0) ? 1u : 0u, ld);
+                      (!first || kk > 0) ? 1u : 0u, ldm);
         }
       };
       if constexpr (kSplit) {

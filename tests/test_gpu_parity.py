@@ -264,3 +264,47 @@ def test_c5_needle_group_is_routed(c5_inputs, depth):
     # and the whole final block (sets, scores, attention output) matches the oracle on the planted input
     rep = parity.check_against_oracle(w, q, kk, v, p, buf, [(0, 0), (0, 3)], [last - 1, last])
     parity.assert_report(rep, w, 4)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the persistent S4 kernel across MANY items per CTA: every block of every slice against the oracle.  The grid is one
+# CTA per SM (148), so n_items >= 4 x 148 makes every CTA walk at least four items through the phase bits, the
+# double-buffered key lists and the pre-issued next-item Q K^T.  items = B * Hkv * n_b * ceil(ceil(G/2)/2).
+# ---------------------------------------------------------------------------------------------------------------
+MULTI_ITEM = [
+    # name,            B, N,    Hq, Hkv, D,   base, Kc, Kg, F, L   -> items (per-CTA items at 148 CTAs)
+    ("mi_g8_d128",     2, 8192, 32, 4, 128, 1e6, 6, 24, 1, 1),   # 2*4*128*2 = 2048 (13.8): <128, split 0, pad 0>
+    ("mi_g1_d64",      4, 4096, 8, 8, 64, 1e4, 8, 20, 1, 1),     # 4*8*64    = 2048 (13.8): <64, split 1, pad 1>
+    ("mi_g3_d64",      2, 8192, 12, 4, 64, 1e4, 8, 20, 1, 1),    # 2*4*128   = 1024 (6.9):  <64, split 0, pad 1>
+    ("mi_g2_d128",     2, 8192, 8, 4, 128, 1e6, 6, 24, 1, 2),    # 2*4*128   = 1024 (6.9):  <128, split 1, pad 1>
+    ("mi_g4_d64",      2, 8192, 16, 4, 64, 1e4, 6, 24, 2, 1),    # 2*4*128   = 1024 (6.9):  <64, split 0, pad 0>
+    # the paper's SmallLM head layout at its own head_dim (hidden 384, 6 query / 2 KV heads -> D 64,
+    # G 3) at its speed-test length (12,288 tokens)
+    ("smalllm_6_2",    2, 12288, 6, 2, 64, 1e4, 16, 32, 1, 1),   # 2*2*192   = 768  (5.2):  <64, split 0, pad 1>
+]
+
+
+@pytest.mark.parametrize("cfg", MULTI_ITEM, ids=[c[0] for c in MULTI_ITEM])
+def test_persistent_kernel_many_items_all_blocks(cfg):
+    name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L = cfg
+    w = W.Workload(name, B, N, Hq, Hkv, D, "bf16", base, n_sink=F, n_local=L, topk_chunks=Kc, topk_groups=Kg)
+    G = Hq // Hkv
+    n_items = B * Hkv * w.n_blocks * (((G + 1) // 2 + 1) // 2)
+    assert n_items >= 4 * 148
+    q, k, v = W.generate(w, 21)
+    p, buf = parity.run_gpu(w, q, k, v, attend_impl=ATTEND_TCGEN05)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks * B * Hkv)
+    assert torch.isfinite(buf.out).all() and torch.isfinite(buf.lse).all()
+
+
+@pytest.mark.parametrize("name,slc", [("c4", (0, 2)), ("c5", (0, 1))])
+def test_full_size_whole_slice_parity(name, slc):
+    """BASELINE.json configs[3], [4] at full size in the bench's launch configuration: one whole (batch, kv head)
+    slice -- all 512 / 1,024 query blocks x 8 heads, index sets + out + LSE -- against the oracle (c5: 8,192 items
+    on 148 CTAs = 55 items per CTA; the slice is 2,048 of them)."""
+    w = W.get(name)
+    q, k, v = W.generate(w, 0)
+    p, buf = parity.run_gpu(w, q, k, v)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [slc], np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks)
