@@ -64,12 +64,16 @@ typedef enum { HGA_F32 = 0, HGA_BF16 = 1 } hga_dtype;
 
 /* Which S4 kernel hga_attend launches. */
 typedef enum {
-  HGA_ATTEND_AUTO = 0,    /* bf16 -> tcgen05/TMEM kernel, f32 -> SIMT fp32 kernel */
+  HGA_ATTEND_AUTO = 0,    /* bf16 -> tcgen05/TMEM kernel (HGA_ATTEND_TCGEN05), f32 -> SIMT fp32 kernel */
   HGA_ATTEND_SIMT = 1,    /* fp32 FMA kernel (any io_dtype): the 1e-4 path for fp32 inputs, and a cross-check */
   HGA_ATTEND_TCGEN05 = 2, /* TMA gather + tcgen05.mma with TMEM accumulators (bf16 inputs only): the persistent
                              kernel; falls back to HGA_ATTEND_TCGEN05_ITEM when the key list does not fit in
                              shared memory beside the tiles */
-  HGA_ATTEND_TCGEN05_ITEM = 3 /* the same arithmetic, one (unit, tile pair) per CTA, no cross-item pipelining */
+  HGA_ATTEND_TCGEN05_ITEM = 3, /* the same arithmetic, one (unit, tile pair) per CTA, no cross-item pipelining */
+  HGA_ATTEND_TCGEN05_PAIR = 4  /* one CTA pair (2-CTA cluster, tcgen05.mma.cta_group::2) per (batch, kv head, block)
+                                  unit: bf16, head_dim 128, groups of exactly 8 query heads; HGA_ERR_UNSUPPORTED
+                                  otherwise.  Same results bit for bit as HGA_ATTEND_TCGEN05; measured slower, so
+                                  HGA_ATTEND_AUTO does not pick it */
 } hga_attend_impl;
 
 /*

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_PKG, "libhga.so")
 _lib = None
 
 HGA_F32, HGA_BF16 = 0, 1
-ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM = 0, 1, 2, 3
+ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM, ATTEND_TCGEN05_PAIR = 0, 1, 2, 3, 4
 
 
 class HgaError(RuntimeError):

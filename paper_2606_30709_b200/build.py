@@ -13,7 +13,7 @@ CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(PKG, "build")
 LIB = os.path.join(PKG, "libhga.so")
 
-SOURCES = ["hga_api.cu", "hga_rope_summary.cu", "hga_route.cu", "hga_attend_simt.cu", "hga_attend_tc.cu", "hga_attend_tc2.cu"]
+SOURCES = ["hga_api.cu", "hga_rope_summary.cu", "hga_route.cu", "hga_attend_simt.cu", "hga_attend_tc.cu", "hga_attend_tc2.cu", "hga_attend_pair.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC,

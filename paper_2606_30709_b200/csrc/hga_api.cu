@@ -31,7 +31,7 @@ hga_status validate(const hga_params* p) {
   if (!(p->softmax_scale >= 0.0f) || !isfinite(p->softmax_scale)) return HGA_ERR_INVALID_ARG;
   if (p->io_dtype != HGA_F32 && p->io_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
   if (p->out_dtype != HGA_F32 && p->out_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
-  if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05_ITEM) return HGA_ERR_INVALID_ARG;
+  if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05_PAIR) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod < 0) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod > 0 && (p->rope_pos_mod % p->chunk || p->pos0 % p->chunk)) return HGA_ERR_INVALID_ARG;
   if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
@@ -162,6 +162,10 @@ hga_status hga_route(const hga_params* p, const float* q_pooled, const float* ch
 static hga_status attend_blocks(const Derived& d, int impl, const void* q_rot, const void* k_rot, const void* v,
                                 const int32_t* group_idx, void* out, float* lse, cudaStream_t cs) {
   hga_status st;
+  if (impl == HGA_ATTEND_TCGEN05_PAIR) return launch_attend_pair(d, q_rot, k_rot, v, group_idx, out, lse, cs);
+  // bf16: the persistent single-CTA kernel.  The CTA-pair kernel is correct (bit-identical results) but measured slower
+  // (c5: 1.33 ms against 0.93 ms), so it is opt-in.
+  if (impl == HGA_ATTEND_AUTO) impl = HGA_ATTEND_TCGEN05;
   if (impl == HGA_ATTEND_TCGEN05) {
     st = launch_attend_tc2(d, q_rot, k_rot, v, group_idx, out, lse, cs);
     if (st != HGA_ERR_UNSUPPORTED) return st;
@@ -173,7 +177,7 @@ static hga_status attend_blocks(const Derived& d, int impl, const void* q_rot, c
 
 static hga_status attend_dispatch(const Derived& d, int impl, const void* q_rot, const void* k_rot, const void* v,
                                   const int32_t* group_idx, void* out, float* lse, cudaStream_t cs) {
-  if (impl == HGA_ATTEND_AUTO) impl = d.bf16_io ? HGA_ATTEND_TCGEN05 : HGA_ATTEND_SIMT;
+  if (impl == HGA_ATTEND_AUTO && !d.bf16_io) impl = HGA_ATTEND_SIMT;
   // The tcgen05 kernels work on whole 64-row blocks.  A partial block (decode step, partial append, ragged prompt
   // tail) goes to the SIMT kernel, which masks rows and never reads a token at or past the end of the window.
   const int last = d.jb + d.nj - 1;

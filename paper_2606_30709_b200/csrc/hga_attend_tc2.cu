@@ -34,6 +34,9 @@
 #include <cuda.h>
 #include <math_constants.h>
 
+#include <type_traits>
+
+#include "hga_attend_softmax.cuh"
 #include "hga_common.cuh"
 #include "hga_tc_ptx.cuh"
 
@@ -50,22 +53,14 @@ constexpr int kLoadWarp = 13;
 constexpr int kListWarp = 14;
 constexpr int kTileKeys = 128;  // keys per KV tile (8 pieces of 16)
 constexpr int kPPT = 8;         // pieces per tile
-constexpr float kRescaleThreshold = 8.0f;  // log2 units
 constexpr int kRegsSoftmax = 200, kRegsEpi = 64, kRegsCtl = 48;  // 2*128*200 + 128*64 + 128*48 = 65536
 
-// exp2 on the FMA pipe for pairs p with (p % kEmuPeriod) < kEmuCount
-#ifndef HGA_S4_EMU_PERIOD
-#define HGA_S4_EMU_PERIOD 4
+#ifdef HGA_S4_TRACE
+__device__ long long g_trace[4096];
+#define HGA_TRM(slot) do { if (tron && lane == 0) g_trace[slot] = clock64(); } while (0)
+#else
+#define HGA_TRM(slot) do { } while (0)
 #endif
-#ifndef HGA_S4_EMU_COUNT
-#define HGA_S4_EMU_COUNT 0  // measured at c5 (S4 ms): 0/4 -> 0.987, 1/8 -> 1.033, 1/4 -> 1.063, 3/8 -> 1.097, 1/2 -> 1.144
-#endif
-#ifndef HGA_S4_DIAG
-#define HGA_S4_DIAG 0  // experiments only, bit mask: 1 = no softmax arithmetic, 2 = no MMAs, 4 = no MUFU, 8 = no K/V TMA
-#endif
-constexpr int kDiag = HGA_S4_DIAG;
-constexpr int kEmuPeriod = HGA_S4_EMU_PERIOD;
-constexpr int kEmuCount = HGA_S4_EMU_COUNT;
 
 struct Tc2Params {
   int B, Hq, Hkv, N, n_b, G;
@@ -119,27 +114,6 @@ __device__ __forceinline__ Item decode_item(int it, const Tc2Params& prm) {
   r.mt0 = cu * 2;
   r.nt = min(2, prm.n_mt - r.mt0);
   return r;
-}
-
-// exp2(x) for x <= ~8 evaluated without MUFU: n = round(x), r = x - n in [-0.5, 0.5], 2^r by a degree-3 polynomial
-// (weighted least squares on Chebyshev nodes, max rel. error 7.5e-5), exponent added in the integer domain.
-__device__ __forceinline__ void exp2_poly2(float x0, float x1, float& p0, float& p1) {
-  const float kMagic = 12582912.0f;  // 1.5 * 2^23: adding it rounds to the nearest integer in the low mantissa bits
-  x0 = fmaxf(x0, -125.0f);
-  x1 = fmaxf(x1, -125.0f);
-  const uint64_t x = pack2(x0, x1);
-  const uint64_t magic = pack2(kMagic, kMagic);
-  const uint64_t t = add2(x, magic);
-  const uint64_t nf = add2(t, pack2(-kMagic, -kMagic));
-  const uint64_t r = fma2(nf, pack2(-1.0f, -1.0f), x);
-  uint64_t p = fma2(pack2(0.0551716648042202f, 0.0551716648042202f), r, pack2(0.2426111251115799f, 0.2426111251115799f));
-  p = fma2(p, r, pack2(0.6932609677314758f, 0.6932609677314758f));
-  p = fma2(p, r, pack2(0.9999280571937561f, 0.9999280571937561f));
-  float t0, t1, q0, q1;
-  unpack2(t, t0, t1);
-  unpack2(p, q0, q1);
-  p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
-  p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
 }
 
 // kSplit: one query tile per item (G <= 2), see the MMA issuer.  kPad: some tile holds a padding head (odd G).
@@ -206,7 +180,6 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const uint32_t s_addr = tmem + lane_base + (uint32_t)(t * 128);
     const uint32_t o_addr = tmem + lane_base + (uint32_t)(256 + t * D);
     const float sl2 = prm.scale_log2;
-    const uint64_t sl2x2 = pack2(sl2, sl2);
     uint32_t s_cnt = 0;  // S_FULL completions consumed
     uint32_t n_done = 0; // items this warpgroup has processed
     int k = 0;
@@ -241,98 +214,25 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           }
           continue;
         }
+        long long* tr = nullptr;
+#ifdef HGA_S4_TRACE
+        if (blockIdx.x == 0 && k >= 8 && k < 10 && (warp % 4) == 0 && i < 8) {
+          tr = g_trace + (((k - 8) * 8 + i) * 2 + t) * 8;
+          if (lane == 0) tr[0] = clock64();
+        }
+#endif
         tc_fence_after();
-        uint32_t sr[128];
-        tmem_ld32(s_addr + 0, sr + 0);
-        tmem_ld32(s_addr + 32, sr + 32);
-        tmem_ld32(s_addr + 64, sr + 64);
-        tmem_ld32(s_addr + 96, sr + 96);
-        tmem_wait_ld();
-        if (i == 0) {
-          // causal mask of the current chunk: key column c (< 64) is token j*64 + c
-#pragma unroll
-          for (int c = 1; c < 64; ++c)
-            if (c > r64) sr[c] = __float_as_uint(-CUDART_INF_F);
-        }
-        if (nk < kTileKeys) {
-#pragma unroll
-          for (int c = 16; c < 128; ++c)
-            if (c >= nk) sr[c] = __float_as_uint(-CUDART_INF_F);
-        }
-        float mx0 = max3(__uint_as_float(sr[0]), __uint_as_float(sr[1]), __uint_as_float(sr[2]));
-        float mx1 = max3(__uint_as_float(sr[3]), __uint_as_float(sr[4]), __uint_as_float(sr[5]));
-        float mx2 = max3(__uint_as_float(sr[6]), __uint_as_float(sr[7]), __uint_as_float(sr[8]));
-        float mx3 = max3(__uint_as_float(sr[9]), __uint_as_float(sr[10]), __uint_as_float(sr[11]));
-#pragma unroll
-        for (int c = 12; c < 124; c += 8) {
-          mx0 = max3(mx0, __uint_as_float(sr[c]), __uint_as_float(sr[c + 1]));
-          mx1 = max3(mx1, __uint_as_float(sr[c + 2]), __uint_as_float(sr[c + 3]));
-          mx2 = max3(mx2, __uint_as_float(sr[c + 4]), __uint_as_float(sr[c + 5]));
-          mx3 = max3(mx3, __uint_as_float(sr[c + 6]), __uint_as_float(sr[c + 7]));
-        }
-        mx0 = max3(mx0, __uint_as_float(sr[124]), __uint_as_float(sr[125]));
-        mx1 = max3(mx1, __uint_as_float(sr[126]), __uint_as_float(sr[127]));
-        const float m_new = fmaxf(m_run, fmaxf(max3(mx0, mx1, mx2), mx3));
-        const bool need = (m_new - m_run) * sl2 > kRescaleThreshold;  // first tile: +inf > 8
-        if (__any_sync(0xffffffffu, need)) {
-          float alpha = 1.f;
-          if (need) {
-            alpha = (m_run == -CUDART_INF_F) ? 0.f : fast_exp2((m_run - m_new) * sl2);
-            m_run = m_new;
-            l_run *= alpha;
-          }
-          if (i != i_first) {
-            // O_t is quiescent here: S_FULL(i) was committed after PV(t, i-1)
-#pragma unroll
-            for (int c0 = 0; c0 < D; c0 += 32) {
-              uint32_t orr[32];
-              tmem_ld32(o_addr + c0, orr);
-              tmem_wait_ld();
-#pragma unroll
-              for (int c = 0; c < 32; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
-              tmem_st32(o_addr + c0, orr);
-            }
-          }
-        }
-        const float neg_m = -m_run * sl2;  // finite: the diagonal key of tile 0 is never masked
-        const uint64_t negm2 = pack2(neg_m, neg_m);
-        uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
-#pragma unroll
-        for (int c0 = 0; c0 < 128; c0 += 32) {
-          uint32_t pr[16];
-#pragma unroll
-          for (int c = 0; c < 16; ++c) {
-            const int pi = (c0 / 2 + c);  // pair index 0..63
-            const uint64_t x = fma2(pack2(__uint_as_float(sr[c0 + 2 * c]), __uint_as_float(sr[c0 + 2 * c + 1])), sl2x2, negm2);
-            float x0, x1, p0, p1;
-            unpack2(x, x0, x1);
-            if ((pi % kEmuPeriod) < kEmuCount) {
-              exp2_poly2(x0, x1, p0, p1);
-            } else {
-              p0 = (kDiag & 4) ? x0 * x0 : fast_exp2(x0);
-              p1 = (kDiag & 4) ? x1 * x1 : fast_exp2(x1);
-            }
-            pr[c] = cvt_bf16x2(p0, p1);  // low half = key 2c, high half = key 2c+1
-            if (c & 1) acc1 = add2(acc1, pack2(p0, p1));
-            else acc0 = add2(acc0, pack2(p0, p1));
-          }
-          tmem_st16(s_addr + (uint32_t)(c0 / 2), pr);  // P overlays S (already in registers)
-          if (c0 == 32) {
-            // keys 0..63 of P are in TMEM: their P V starts while the second half is still being exponentiated,
-            // which takes half a P V off the softmax -> P V -> Q K^T -> softmax latency chain of this tile
-            tmem_wait_st();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(BAR(L::PFULL + t));
-          }
-        }
-        float a0, a1;
-        unpack2(add2(acc0, acc1), a0, a1);
-        l_run += a0 + a1;
-        tmem_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(BAR(L::PFULLB + t));
+        softmax_tile<D>(
+            s_addr, o_addr, i == 0, r64, nk, i != i_first, sl2, m_run, l_run,
+            [&] {
+              __syncwarp();
+              if (lane == 0) mbar_arrive(BAR(L::PFULL + t));
+            },
+            [&] {
+              __syncwarp();
+              if (lane == 0) mbar_arrive(BAR(L::PFULLB + t));
+            },
+            tr);
       }
       // ---- item done: hand 1/l to the epilogue warpgroup, write LSE ----------------------------------------------
       mbar_wait(BAR(L::LEMPTY + t), (n_done & 1u) ^ 1u);
@@ -565,6 +465,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // The whole warp runs the control flow convergently (so operands stay warp-uniform and ptxas needs no
       // per-lane broadcast loops); only the tcgen05 instructions themselves are predicated on one elected lane.
       const uint32_t ld = elect_one();
+      const uint32_t tmem_u = uni(tmem);  // warp-uniform for ptxas: descriptors and addresses stay in uniform registers
       const uint32_t ldm = (kDiag & 2) ? 0u : ld;  // MMA issue predicate
       const uint32_t idesc_pv = umma_idesc(128, D, /*b_mn_major=*/true);
       const uint32_t idesc_qk_full = umma_idesc(128, kTileKeys, false);
@@ -572,14 +473,11 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
       constexpr uint32_t kLboK = (16u >> 4) << 16;                      // K-major operands (Q, K)
       constexpr uint32_t kLboV = ((uint32_t)L::kHalfBytes >> 4) << 16;  // MN-major V: next 64 columns
-      uint32_t q_cnt0 = 0, q_cnt1 = 0;    // Q_FULL completions consumed per tile
-      uint32_t p_cnt0 = 0, p_cnt1 = 0;    // P_FULL completions consumed per tile
-      uint32_t oe_cnt0 = 0, oe_cnt1 = 0;  // O_EMPTY waits per tile
       auto issue_qk = [&](int t, int s, int nkeys) {
         const uint32_t idesc = nkeys == kTileKeys ? idesc_qk_full : umma_idesc(128, nkeys, false);
         const uint32_t qa = ((sbase + L::kQ + t * L::kTileBytes) & 0x3FFFFu) >> 4;
         const uint32_t ka = ((sbase + L::kK + s * L::kTileBytes) & 0x3FFFFu) >> 4;
-        const uint32_t d = tmem + (uint32_t)(t * 128);
+        const uint32_t d = tmem_u + (uint32_t)(t * 128);
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t o = (uint32_t)((kk / 4) * L::kHalfBytes + (kk % 4) * 32) >> 4;
@@ -588,8 +486,8 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       };
       auto issue_pv = [&](int t, int s, int kk0, int kk1, bool first) {
         const uint32_t va = ((sbase + L::kV + s * L::kTileBytes) & 0x3FFFFu) >> 4;
-        const uint32_t d = tmem + (uint32_t)(256 + t * D);
-        const uint32_t a = tmem + (uint32_t)(t * 128);
+        const uint32_t d = tmem_u + (uint32_t)(256 + t * D);
+        const uint32_t a = tmem_u + (uint32_t)(t * 128);
         // A: P_t columns [8kk, 8kk+8) (16 bf16 keys); B: V rows 16kk..16kk+15, MN-major
         if (kk1 - kk0 == kPPT / 2) {
 #pragma unroll
@@ -633,7 +531,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           const int buf = k & 1;
           const bool has_next = it + (int)gridDim.x < prm.n_items;
           mbar_wait(BAR(L::LISTFULL + buf), (uint32_t)(k >> 1) & 1u);
-          const int n_pieces = s_np[buf];
+          const int n_pieces = uni(s_np[buf]);
           const int n_tiles = (n_pieces + kPPT - 1) / kPPT;
           auto nkeys_of = [&](int u) { return min(kPPT, n_pieces - u * kPPT) * 16; };
           auto st_of = [&](int u) { return (int)((base + (uint32_t)u) % L::kStages); };
@@ -670,7 +568,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
               if (has_next) {
                 // S_t is free once this P V has run: queue the next item's first Q K^T of this tile right behind it
                 mbar_wait(BAR(L::LISTFULL + (buf ^ 1)), (uint32_t)((k + 1) >> 1) & 1u);
-                first_qk(t, s_np[buf ^ 1], base + (uint32_t)n_tiles);
+                first_qk(t, uni(s_np[buf ^ 1]), base + (uint32_t)n_tiles);
                 pre[t] = true;
               }
             }
@@ -687,24 +585,77 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
         }
       }
+      // General case (two query tiles per item).  The issuer warp is a serial instruction stream, and at 64 cycles
+      // per MMA it -- not the tensor pipe -- sets the pace as soon as it spends more than that per instruction
+      // (descriptor words moved from vector to uniform registers, ~100 cycles per barrier wait): measured 3,300
+      // cycles per key-tile step against 2,048 of MMA work.  So the key-tile step is instantiated once per ring
+      // stage: the tile and stage indices are compile-time constants and every descriptor is a constant offset from
+      // the (uniform) shared-memory base.
       uint32_t step = 0;  // K/V tiles consumed so far: tile `step` lives in stage step % kStages
       int k = 0;
       int it = kSplit ? prm.n_items : blockIdx.x;  // split mode is handled above
       int n_pieces = 0, nt = 0;
+      uint32_t q_cnt[2] = {0, 0}, p_cnt[2] = {0, 0}, oe_cnt[2] = {0, 0};
+      const uint32_t sb4 = (sbase & 0x3FFFFu) >> 4;  // tile bases are 1024-byte aligned: offsets add without carry
+      auto qk = [&](auto T, auto S, int nkeys) {
+        constexpr int t = decltype(T)::value, st = decltype(S)::value;
+        const uint32_t idesc = nkeys == kTileKeys ? idesc_qk_full : umma_idesc(128, nkeys, false);
+        const uint32_t d = tmem_u + (uint32_t)(t * 128);
+#pragma unroll
+        for (int kk = 0; kk < D / 16; ++kk) {
+          constexpr uint32_t kZero = 0;
+          const uint32_t o = (uint32_t)((kk / 4) * L::kHalfBytes + (kk % 4) * 32) >> 4;
+          const uint32_t qo = ((uint32_t)(L::kQ + t * L::kTileBytes) >> 4) + o + kLboK + kZero;
+          const uint32_t ko = ((uint32_t)(L::kK + st * L::kTileBytes) >> 4) + o + kLboK;
+          umma_ss_e(d, make_desc(sb4 + qo, kDescHi), make_desc(sb4 + ko, kDescHi), idesc, kk > 0 ? 1u : 0u, ldm);
+        }
+      };
+      auto pv = [&](auto T, auto S, int kk0, int kk1, bool first) {
+        constexpr int t = decltype(T)::value, st = decltype(S)::value;
+        const uint32_t d = tmem_u + (uint32_t)(256 + t * D);
+        const uint32_t a = tmem_u + (uint32_t)(t * 128);
+        // A: P_t columns [8kk, 8kk+8) (16 bf16 keys); B: V rows 16kk..16kk+15, MN-major
+        auto one = [&](int kk, uint32_t acc) {
+          const uint32_t vo = ((uint32_t)(L::kV + st * L::kTileBytes + kk * 16 * 128) >> 4) + kLboV;
+          umma_ts_e(d, a + (uint32_t)(kk * 8), make_desc(sb4 + vo, kDescHi), idesc_pv, acc, ldm);
+        };
+        if (kk1 - kk0 == kPPT / 2) {  // a whole half tile: no per-instruction branches
+          if (kk0 == 0) {
+            one(0, first ? 0u : 1u);
+            one(1, 1u);
+            one(2, 1u);
+            one(3, 1u);
+          } else {
+            one(4, 1u);
+            one(5, 1u);
+            one(6, 1u);
+            one(7, 1u);
+          }
+        } else {
+#pragma unroll
+          for (int kk = 0; kk < kPPT; ++kk)
+            if (kk >= kk0 && kk < kk1) one(kk, (!first || kk > 0) ? 1u : 0u);
+        }
+      };
       if (it < prm.n_items) {
         mbar_wait(BAR(L::LISTFULL + 0), 0);
-        n_pieces = s_np[0];
+        n_pieces = uni(s_np[0]);
         nt = decode_item(it, prm).nt;
         // first Q K^T of the first item
         mbar_wait(BAR(L::KFULL + 0), 0);
-        for (int t = 0; t < nt; ++t) {
-          mbar_wait(BAR(L::QFULL + t), 0);
-          if (t == 0) ++q_cnt0; else ++q_cnt1;
-          tc_fence_after();
-          issue_qk(t, 0, min(kPPT, n_pieces) * 16);
-          umma_commit_e(BAR(L::SFULL + t), ld);
-          if (n_pieces <= kPPT) umma_commit_e(BAR(L::QEMPTY + t), ld);
-        }
+        auto first_qk = [&](auto T) {
+          constexpr int t = decltype(T)::value;
+          if (t < nt) {
+            mbar_wait(BAR(L::QFULL + t), 0);
+            ++q_cnt[t];
+            tc_fence_after();
+            qk(T, std::integral_constant<int, 0>{}, min(kPPT, n_pieces) * 16);
+            umma_commit_e(BAR(L::SFULL + t), ld);
+            if (n_pieces <= kPPT) umma_commit_e(BAR(L::QEMPTY + t), ld);
+          }
+        };
+        first_qk(std::integral_constant<int, 0>{});
+        first_qk(std::integral_constant<int, 1>{});
         umma_commit_e(BAR(L::KEMPTY + 0), ld);
       }
       for (; it < prm.n_items; it += gridDim.x, ++k) {
@@ -714,8 +665,6 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         const bool has_next = it_next < prm.n_items;
         int n_pieces_next = 0, nt_next = 0;
         for (int i = 0; i < n_tiles; ++i, ++step) {
-          const int vs = (int)(step % L::kStages);
-          const int ks = (int)((step + 1) % L::kStages);
           const bool last = (i + 1 == n_tiles);
           const bool more = !last || has_next;  // another Q K^T follows this tile's P V
           int nkeys_next = 0, n_tiles_after = 0;
@@ -724,48 +673,71 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             n_tiles_after = n_tiles - (i + 2);
           } else if (has_next) {
             mbar_wait(BAR(L::LISTFULL + (buf ^ 1)), (uint32_t)((k + 1) >> 1) & 1u);
-            n_pieces_next = s_np[buf ^ 1];
+            n_pieces_next = uni(s_np[buf ^ 1]);
             nt_next = decode_item(it_next, prm).nt;
             nkeys_next = min(kPPT, n_pieces_next) * 16;
             n_tiles_after = (n_pieces_next + kPPT - 1) / kPPT - 1;
           }
           const int nkeys = min(kPPT, n_pieces - i * kPPT) * 16;
-          mbar_wait(BAR(L::VFULL + vs), (step / L::kStages) & 1u);
-          if (more) mbar_wait(BAR(L::KFULL + ks), ((step + 1) / L::kStages) & 1u);
           const int nt_qk = last ? nt_next : nt;
-#pragma unroll
-          for (int t = 0; t < 2; ++t) {
-            uint32_t& p_cnt = t == 0 ? p_cnt0 : p_cnt1;
-            uint32_t& oe_cnt = t == 0 ? oe_cnt0 : oe_cnt1;
-            uint32_t& q_cnt = t == 0 ? q_cnt0 : q_cnt1;
-            if (t < nt) {
-              mbar_wait(BAR(L::PFULL + t), p_cnt & 1u);  // keys 0..63 of P_t
-              if (i == 0) {
-                // the epilogue has drained the previous item's O_t
-                mbar_wait(BAR(L::OEMPTY + t), (oe_cnt & 1u) ^ 1u);
-                ++oe_cnt;
-              }
-              tc_fence_after();
-              issue_pv(t, vs, 0, min(nkeys / 16, kPPT / 2), i == 0);
-              mbar_wait(BAR(L::PFULLB + t), p_cnt & 1u);  // keys 64..127
-              ++p_cnt;
-              tc_fence_after();
-              issue_pv(t, vs, kPPT / 2, nkeys / 16, false);
-              if (last) umma_commit_e(BAR(L::OFULL + t), ld);
-            }
-            if (more && t < nt_qk) {
-              if (last) {
-                mbar_wait(BAR(L::QFULL + t), q_cnt & 1u);
-                ++q_cnt;
+          const uint32_t v_ph = (step / L::kStages) & 1u, k_ph = ((step + 1) / L::kStages) & 1u;
+          // one key-tile step with the V tile in stage VS and the next K tile in stage KS
+          auto tile_step = [&](auto VS) {
+            constexpr int vs = decltype(VS)::value, ks = (vs + 1) % L::kStages;
+            using KS = std::integral_constant<int, ks>;
+            mbar_wait(BAR(L::VFULL + vs), v_ph);
+            if (more) mbar_wait(BAR(L::KFULL + ks), k_ph);
+            auto one = [&](auto T) {
+              constexpr int t = decltype(T)::value;
+              const bool tron = blockIdx.x == 0 && k >= 8 && k < 10 && i < 8;
+              const int trs = 1024 + (((k - 8) * 8 + i) * 2 + t) * 8;
+              (void)tron;
+              (void)trs;
+              if (t < nt) {
+                mbar_wait(BAR(L::PFULL + t), p_cnt[t] & 1u);  // keys 0..63 of P_t
+                HGA_TRM(trs + 0);
+                if (i == 0) {
+                  // the epilogue has drained the previous item's O_t
+                  mbar_wait(BAR(L::OEMPTY + t), (oe_cnt[t] & 1u) ^ 1u);
+                  ++oe_cnt[t];
+                }
                 tc_fence_after();
+                pv(T, VS, 0, min(nkeys / 16, kPPT / 2), i == 0);
+                HGA_TRM(trs + 1);
+                mbar_wait(BAR(L::PFULLB + t), p_cnt[t] & 1u);  // keys 64..127
+                HGA_TRM(trs + 2);
+                ++p_cnt[t];
+                tc_fence_after();
+                pv(T, VS, kPPT / 2, nkeys / 16, false);
+                if (last) umma_commit_e(BAR(L::OFULL + t), ld);
               }
-              issue_qk(t, ks, nkeys_next);
-              umma_commit_e(BAR(L::SFULL + t), ld);
-              if (n_tiles_after == 0) umma_commit_e(BAR(L::QEMPTY + t), ld);  // that was the item's last Q K^T
-            }
+              if (more && t < nt_qk) {
+                if (last) {
+                  mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+                  ++q_cnt[t];
+                  tc_fence_after();
+                }
+                qk(T, KS{}, nkeys_next);
+                umma_commit_e(BAR(L::SFULL + t), ld);
+                if (n_tiles_after == 0) umma_commit_e(BAR(L::QEMPTY + t), ld);  // that was the item's last Q K^T
+              }
+              HGA_TRM(trs + 3);
+            };
+            one(std::integral_constant<int, 0>{});
+            one(std::integral_constant<int, 1>{});
+            umma_commit_e(BAR(L::VEMPTY + vs), ld);
+            if (more) umma_commit_e(BAR(L::KEMPTY + ks), ld);
+          };
+          const uint32_t vsi = step % L::kStages;
+          if constexpr (L::kStages == 2) {
+            if (vsi == 0) tile_step(std::integral_constant<int, 0>{});
+            else tile_step(std::integral_constant<int, 1>{});
+          } else {
+            if (vsi == 0) tile_step(std::integral_constant<int, 0>{});
+            else if (vsi == 1) tile_step(std::integral_constant<int, 1>{});
+            else if (vsi == 2) tile_step(std::integral_constant<int, 2>{});
+            else tile_step(std::integral_constant<int, 3>{});
           }
-          umma_commit_e(BAR(L::VEMPTY + vs), ld);
-          if (more) umma_commit_e(BAR(L::KEMPTY + ks), ld);
         }
         if (lane == 0) mbar_arrive(BAR(L::LISTEMPTY + buf));
         n_pieces = n_pieces_next;
@@ -824,6 +796,12 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
 }
 
 }  // namespace
+
+#ifdef HGA_S4_TRACE
+extern "C" __attribute__((visibility("default"))) int hga_debug_trace(long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(long long) * 4096);
+}
+#endif
 
 // Returns HGA_ERR_UNSUPPORTED when the key list does not fit beside the tiles (the caller falls back to the
 // one-item-per-CTA kernel).

@@ -93,6 +93,8 @@ hga_status launch_attend_simt(const Derived& d, const void* q, const void* k, co
                               void* out, float* lse, cudaStream_t s);
 hga_status launch_attend_tc2(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                              void* out, float* lse, cudaStream_t s);
+hga_status launch_attend_pair(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
+                              void* out, float* lse, cudaStream_t s);
 hga_status launch_attend_tc(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                             void* out, float* lse, cudaStream_t s);
 

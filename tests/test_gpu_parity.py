@@ -11,8 +11,8 @@ import torch
 import hga_workloads as W
 import oracle
 import paper_2606_30709_b200 as hga
-from paper_2606_30709_b200.binding import (ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM, HGA_BF16,
-                                             HGA_F32)
+from paper_2606_30709_b200.binding import (ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM,
+                                             ATTEND_TCGEN05_PAIR, HGA_BF16, HGA_F32)
 
 import parity
 
@@ -296,6 +296,11 @@ def test_persistent_kernel_many_items_all_blocks(cfg):
     rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
     parity.assert_report(rep, w, w.n_blocks * B * Hkv)
     assert torch.isfinite(buf.out).all() and torch.isfinite(buf.lse).all()
+    if G == 8 and D == 128:  # the CTA-pair kernel: 1,024 units on 74 pairs = 13.8 units per pair
+        p2, buf2 = parity.run_gpu(w, q, k, v, attend_impl=ATTEND_TCGEN05_PAIR)
+        rep = parity.check_against_oracle(w, q, k, v, p2, buf2, _all_slices(w), np.arange(w.n_blocks))
+        parity.assert_report(rep, w, w.n_blocks * B * Hkv)
+        assert torch.isfinite(buf2.out).all() and torch.isfinite(buf2.lse).all()
 
 
 @pytest.mark.parametrize("name,slc", [("c4", (0, 2)), ("c5", (0, 1))])
@@ -308,3 +313,49 @@ def test_full_size_whole_slice_parity(name, slc):
     p, buf = parity.run_gpu(w, q, k, v)
     rep = parity.check_against_oracle(w, q, k, v, p, buf, [slc], np.arange(w.n_blocks))
     parity.assert_report(rep, w, w.n_blocks)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the CTA-pair S4 kernel (tcgen05.mma.cta_group::2; bf16, D 128, G 8): every block against the oracle.  The last key
+# tile of a unit holds np = n_pieces % 8 sixteen-key pieces, split ceil(np/2) / floor(np/2) between the two CTAs:
+# the cases cover np = 1..7 and 0 (full), the windows F/L in {0..3}, 32-token groups, and bf16 output.
+# ---------------------------------------------------------------------------------------------------------------
+PAIR = [
+    # name,        B, N,    Hq, Hkv, Kc, Kg, F, L, group   steady-state pieces = 4*(F + max(L,1) + 1) + Kg*group/16
+    ("np4",        1, 2048, 16, 2, 6, 24, 1, 1, 16),   # 36 -> 4 full tiles + 4 pieces
+    ("np1",        1, 2048, 16, 2, 6, 21, 1, 1, 16),   # 33 -> np 1: the peer CTA holds no key of the last tile
+    ("np2",        1, 2048, 8, 1, 6, 22, 1, 1, 16),    # 34
+    ("np3",        1, 2048, 8, 1, 6, 23, 1, 1, 16),    # 35
+    ("np5",        1, 2048, 8, 1, 8, 25, 1, 1, 16),    # 37
+    ("np6_f0l0",   1, 2048, 8, 1, 8, 30, 0, 0, 16),    # 8 + 30 = 38
+    ("np7_f2l3",   1, 2048, 8, 1, 8, 31, 2, 3, 16),    # 24 + 31 = 55 -> 6 tiles + 7
+    ("np0_gs32",   2, 2048, 8, 1, 6, 10, 1, 1, 32),    # 12 + 20 = 32 -> exactly 4 tiles
+    ("tiny_lists", 1, 1024, 16, 2, 1, 2, 1, 1, 16),    # 14 pieces: 2 tiles
+]
+
+
+@pytest.mark.parametrize("out_dtype", [HGA_F32, HGA_BF16], ids=["f32out", "bf16out"])
+@pytest.mark.parametrize("cfg", PAIR, ids=[c[0] for c in PAIR])
+def test_pair_kernel_full_parity(cfg, out_dtype):
+    name, B, N, Hq, Hkv, Kc, Kg, F, L, gs = cfg
+    w = W.Workload("pair_" + name, B, N, Hq, Hkv, 128, "bf16", 1e6, group=gs, n_sink=F, n_local=L, topk_chunks=Kc,
+                   topk_groups=Kg, n_clusters=8)
+    q, k, v = W.generate(w, 17)
+    p, buf = parity.run_gpu(w, q, k, v, attend_impl=ATTEND_TCGEN05_PAIR, out_dtype=out_dtype)
+    if out_dtype == HGA_F32:
+        rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
+        parity.assert_report(rep, w, w.n_blocks * B * Hkv)
+    # the same arithmetic in the same order as the single-CTA kernel (same MMA shapes per row, same softmax code)
+    p1, buf1 = parity.run_gpu(w, q, k, v, attend_impl=ATTEND_TCGEN05, out_dtype=out_dtype)
+    assert (buf.out.float() - buf1.out.float()).abs().max().item() <= (2e-2 if out_dtype == HGA_F32 else 2.0 ** -6)
+    assert (buf.lse - buf1.lse).abs().max().item() <= 2e-2
+
+
+def test_pair_kernel_rejects_other_shapes():
+    w = W.Workload("pair_bad", 1, 512, 4, 2, 128, "bf16", 1e6, topk_chunks=2, topk_groups=4)
+    p = hga.params_from_workload(w, attend_impl=ATTEND_TCGEN05_PAIR)
+    x = torch.zeros((1, 4, 512, 128), dtype=torch.bfloat16, device="cuda")
+    kv = torch.zeros((1, 2, 512, 128), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(hga.HgaError) as e:
+        hga.hga_attend(p, x, kv, kv, torch.full((1, 2, 8, 4), -1, dtype=torch.int32, device="cuda"))
+    assert e.value.code == 2
