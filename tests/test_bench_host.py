@@ -62,7 +62,7 @@ def test_reference_arm_under_torchrun_rank0_prints_others_exit_0():
     port = _free_port()
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
            "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
-           "--steps", "1", "--warmup", "0", "--workload", "c1", "--ref-blocks", "4"]
+           "--steps", "1", "--warmup", "0", "--workload", "c1"]
     res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert res.returncode == 0, res.stderr[-2000:]
     lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
@@ -86,6 +86,11 @@ def test_algorithmic_work_matches_survey_figures():
     assert a4["s4_flops"] == pytest.approx(0.641e12, rel=0.01)
     last = 4 * 128 * (64 * 8) * (48 * 16 + 3 * 64)
     assert last == 4 * 128 * 512 * 960
+    # compulsory S4 DRAM bytes (c5 1208 MB with bf16 output; fp32 output adds another |Q|): Q + O + K + V
+    assert a5["s4_bytes"] == 537e6 * 0 + (65536 * 32 * 128) * (2 + 4) + 2 * (65536 * 4 * 128) * 2
+    assert a5["s4_bytes_gathered"] > 2 * a5["s4_bytes"]  # the per-block re-gathers are L2 traffic, not DRAM
+    # useful FLOPs exclude the masked half of the causal chunk: 63/128 of one 64-key chunk per block
+    assert a5["s4_flops_useful"] == a5["s4_flops"] - 4 * 128 * 32 * 1024 * (64 * 63 // 2)
 
 
 def test_peaks_loader_falls_back_to_the_profiling_guide_numbers(tmp_path, monkeypatch):
