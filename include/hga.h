@@ -221,11 +221,17 @@ HGA_API hga_status hga_prefill(const hga_params* p, const hga_buffers* buf, void
  *     decode token routes with its own pooled query) against the closed chunks before it (S2, S3); results go to row
  *     j = t / chunk of q_pooled / chunk_idx / group_idx / ... (overwriting what an earlier step of the same block left);
  *   - attends (S4): writes the out / lse rows of the window and no others.  Whole 64-row blocks go to the kernel
- *     hga_attend would pick; a partial block (a window that starts or ends inside a chunk) goes to the fp32 SIMT kernel.
+ *     hga_attend would pick; a partial block (a window that starts or ends inside a chunk) goes to the fp32 kernels --
+ *     steps of up to 4 query rows (decode, short appends) to attend_rows_kernel (key list split over 8 warps, online
+ *     softmax per warp, partial results merged), longer partial blocks to the row-masked SIMT tile kernel.
  *     A window that starts inside a chunk must stay inside that chunk (one step of the active chunk).
+ * In-place RoPE: q_rot may alias q_raw for any window.  k_rot may alias k_raw ONLY for chunk-aligned windows
+ * (t_begin and t_end multiples of chunk): a step that closes a chunk summarises the whole chunk from k_raw, and with
+ * the alias earlier partial steps would already have replaced its first rows by rotated keys.
  * Values at positions >= t_end never influence a result and nothing there is written: the future part of the cache
  * may be uninitialised (even NaN).  A chunk is summarised only by the call whose window closes it.
- * Errors: HGA_ERR_INVALID_ARG for an empty/out-of-range window or one that starts inside a chunk and leaves it.
+ * Errors: HGA_ERR_INVALID_ARG for an empty/out-of-range window, one that starts inside a chunk and leaves it, or
+ * k_rot == k_raw with a window that is not chunk-aligned.
  */
 HGA_API hga_status hga_prefill_window(const hga_params* p, const hga_buffers* buf, int64_t t_begin, int64_t t_end,
                                       void* stream);

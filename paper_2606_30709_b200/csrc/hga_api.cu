@@ -220,6 +220,9 @@ static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* 
   if (t_begin < 0 || t_begin >= t_end || t_end > d.N) return HGA_ERR_INVALID_ARG;
   // a window that starts inside a chunk stays inside it (one step of the active chunk)
   if (t_begin % kChunk != 0 && (t_begin / kChunk) != ((t_end - 1) / kChunk)) return HGA_ERR_INVALID_ARG;
+  // In-place K (k_rot == k_raw) is only sound for chunk-aligned steps: a step that closes a chunk summarises the whole
+  // 64-token tile from k_raw, and earlier partial steps would already have overwritten its first rows with rotated values.
+  if (b->k_rot == b->k_raw && (t_begin % kChunk != 0 || t_end % kChunk != 0)) return HGA_ERR_INVALID_ARG;
   d.tw0 = t_begin; d.tw1 = t_end;
   d.jb = (int)(t_begin / kChunk);
   d.nj = (int)((t_end + kChunk - 1) / kChunk) - d.jb;
@@ -372,7 +375,7 @@ hga_status hga_host_plan_create(const hga_params* p, hga_host_plan** out_plan) {
   return HGA_OK;
 }
 
-hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k_host, const void* v_host,
+static hga_status host_prefill_body(hga_host_plan* pl, const void* q_host, const void* k_host, const void* v_host,
                             void* out_host, int32_t* group_idx_host, float* lse_host) {
   if (!pl || !q_host || !k_host || !v_host || !out_host) return HGA_ERR_INVALID_ARG;
   const Derived& d = pl->d;
@@ -434,6 +437,18 @@ hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k
   HGA_CUDA_OK(cudaStreamSynchronize(pl->s_out));
   HGA_CUDA_OK(cudaStreamSynchronize(pl->stream));
   return HGA_OK;
+}
+
+hga_status hga_host_prefill(hga_host_plan* pl, const void* q_host, const void* k_host, const void* v_host,
+                            void* out_host, int32_t* group_idx_host, float* lse_host) {
+  const hga_status st = host_prefill_body(pl, q_host, k_host, v_host, out_host, group_idx_host, lse_host);
+  if (st != HGA_OK && pl) {
+    // copies from / to caller-owned host buffers may still be in flight: drain them before handing control back
+    cudaStreamSynchronize(pl->s_in);
+    cudaStreamSynchronize(pl->stream);
+    cudaStreamSynchronize(pl->s_out);
+  }
+  return st;
 }
 
 void hga_host_plan_destroy(hga_host_plan* pl) {

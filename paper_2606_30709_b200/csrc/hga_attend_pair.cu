@@ -541,9 +541,8 @@ hga_status launch_attend_pair(const Derived& d, const void* q, const void* k, co
   ok = ok && (d.bf16_out ? make_map_2d(&tmO, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, out, q_rows, kD, 64, 32)
                          : make_map_2d(&tmO, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, out, q_rows, kD, 32, 32));
   if (!ok) return HGA_ERR_CUDA;
-  int dev = 0, n_sm = 0;
-  HGA_CUDA_OK(cudaGetDevice(&dev));
-  HGA_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  const int n_sm = current_sm_count();
+  if (n_sm <= 0) return HGA_ERR_CUDA;
   HGA_CUDA_OK(cudaFuncSetAttribute(attend_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int n_pairs = (int)(n_items < n_sm / 2 ? n_items : n_sm / 2);
   attend_pair_kernel<<<2 * n_pairs, kThreads, smem, s>>>(tmQ, tmK, tmV, tmO, group_idx, lse, prm);

@@ -781,12 +781,8 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
   ok = ok && (d.bf16_out ? make_map_2d(&tmO, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, out, q_rows, D, 64, 32)
                          : make_map_2d(&tmO, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, out, q_rows, D, 32, 32));
   if (!ok) return HGA_ERR_CUDA;
-  static int n_sm = 0;
-  if (n_sm == 0) {
-    int dev = 0;
-    HGA_CUDA_OK(cudaGetDevice(&dev));
-    HGA_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-  }
+  const int n_sm = current_sm_count();
+  if (n_sm <= 0) return HGA_ERR_CUDA;
   auto kern = prm.split ? attend_tc2_kernel<D, true, true>
                         : (d.G % 2 ? attend_tc2_kernel<D, false, true> : attend_tc2_kernel<D, false, false>);
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -41,6 +41,15 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f);
     if (_e != cudaSuccess) return HGA_ERR_CUDA; \
   } while (0)
 
+// SM count of the CURRENT device (queried per call: a process may use more than one device type or MIG slice, and a
+// cached static would also be a data race between concurrent callers).  Returns 0 on failure.
+inline int current_sm_count() {
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+  return n;
+}
+
 inline hga_status launch_status() { return cudaGetLastError() == cudaSuccess ? HGA_OK : HGA_ERR_CUDA; }
 
 // ---- element I/O helpers -------------------------------------------------------------------------------------

@@ -338,12 +338,8 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
 template <typename T, int D>
 hga_status launch_stream_t(const RopeFreq& f, RsParams p, long long rows, cudaStream_t s) {
   using C = RsCfg<T, D>;
-  static int n_sm = 0;
-  if (n_sm == 0) {
-    int dev = 0;
-    HGA_CUDA_OK(cudaGetDevice(&dev));
-    HGA_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-  }
+  const int n_sm = current_sm_count();
+  if (n_sm <= 0) return HGA_ERR_CUDA;
   p.tpr = p.HK + p.HQ;
   p.total_tiles = rows * p.tpr;
   const long long units = rows * (p.HK + (p.HQ ? p.HQ / p.PG : 0));

@@ -8,7 +8,6 @@ Outputs: max-abs <= 1e-4 (fp32 inputs) / 2e-2 (bf16 inputs, fp32 accumulation).
 from __future__ import annotations
 
 import dataclasses
-import os
 
 import numpy as np
 import torch
@@ -69,8 +68,6 @@ def check_lists_wellformed(idx: np.ndarray, cnt: np.ndarray):
 
 def run_gpu(w: W.Workload, q, k, v, attend_impl=hga.binding.ATTEND_AUTO, out_dtype=hga.binding.HGA_F32, **over):
     """Whole path through hga_prefill.  q,k,v: numpy fp32 arrays from hga_workloads."""
-    if attend_impl == hga.binding.ATTEND_AUTO and os.environ.get("HGA_TEST_ATTEND_IMPL"):  # debugging aid
-        attend_impl = int(os.environ["HGA_TEST_ATTEND_IMPL"])
     p = hga.params_from_workload(w, out_dtype=out_dtype, attend_impl=attend_impl)
     if over:
         p = p.replace(**over)
@@ -112,6 +109,12 @@ def check_against_oracle(w: W.Workload, q, k, v, p, buf, slices, blocks, check_i
             worst["group_sum"] = max(worst["group_sum"], float(np.abs(gs_ - r.group_sum).max()))
             qp = buf.q_pooled[b, kh].cpu().numpy().astype(np.float64)[blocks]
             worst["pooled"] = max(worst["pooled"], float(np.abs(qp - r.q_pooled).max()))
+            # rotated queries of the sampled blocks against O1 rounded to the I/O dtype (one storage rounding apart)
+            for j in blocks[:: max(1, len(blocks) // 8)]:
+                qo = oracle.round_io(oracle.rope(q[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C], op.pos0 + j * C, op.base,
+                                                 op.pos_mod), op.io_bf16)
+                qg = buf.q_rot[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C].float().cpu().numpy().astype(np.float64)
+                worst["q_rot"] = max(worst["q_rot"], float(np.abs(qg - qo).max()))
         g_out = buf.out[b, kh * G:(kh + 1) * G].float().cpu().numpy().astype(np.float64)  # [G,N,D]
         g_lse = buf.lse[b, kh * G:(kh + 1) * G].cpu().numpy().astype(np.float64)
         kv64 = v[b, kh].astype(np.float64)
@@ -165,3 +168,4 @@ def assert_report(rep, w: W.Workload, n_checked: int, score_tol: float = 1e-6):
     assert wst["score"] <= score_tol, rep
     # rotated keys: one storage rounding apart at most (fp32: ~1e-6 abs; bf16: 1 ulp of values up to ~8 -> 2^-4)
     assert wst["k_rot"] <= (4e-6 if w.dtype == "f32" else 0.0625), rep
+    assert wst["q_rot"] <= (4e-6 if w.dtype == "f32" else 0.0625), rep
