@@ -21,6 +21,8 @@ from .hga_oracle import (  # noqa: F401
     rope,
     round_io,
     route_chunks,
+    route_chunks_max,
+    route_groups_max,
     route_groups,
     step,
     summaries,

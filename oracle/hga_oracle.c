@@ -60,6 +60,12 @@ typedef struct {
                          65536); 0 = off.  Reading R18: every position that enters a rotation is wrapped, and
                          pos_mod and pos0 must be multiples of C so that no span straddles a wrap (its "middle
                          position" R2 is then wrapped start + (S-1)/2); the routing algorithm is unchanged. */
+  int32_t route_max;  /* N3 variant (R4's alternative): 0 = a block's score of a candidate is the
+                         dot product with the POOLED query (mean of per-query scores); 1 = the MAX over the block's
+                         64*G per-query scores.  Reading R19: the per-query scores use the rotated queries as STORED
+                         (rounded to the I/O dtype, the only per-query rotated form the method keeps, R7); the pooled
+                         query is still returned.  Everything downstream (top-k, ties, order) is unchanged. */
+  int32_t pad_;
 } hga_oracle_params;
 
 int hga_oracle_max_threads(void) {
@@ -314,6 +320,70 @@ int hga_oracle_route_groups(const double* qbar_j, const double* S_g, int D, int 
 }
 
 /* ------------------------------------------------------------------------------------------------ */
+/* N3  R4's alternative: max over per-query scores (PAPER.md:33, 45, 97 leave open how the 64*G queries of a   */
+/*     block become one score).  q_rows [n_rows, D] are the block's rotated queries (all heads of the GQA      */
+/*     group); score(c) = max_r q_rows[r] . S[c].  Candidate sets, budgets, ties and output order are those of */
+/*     O4 / O5.                                                                                              */
+/* ------------------------------------------------------------------------------------------------ */
+static double max_dot(const double* q_rows, int n_rows, const double* s, int D) {
+  double best = -INFINITY;
+  for (int r = 0; r < n_rows; ++r) {
+    double v = dot(q_rows + (size_t)r * D, s, D);
+    if (v > best) best = v;
+  }
+  return best;
+}
+
+int hga_oracle_route_chunks_max(const double* q_rows, int n_rows, const double* S_c, int n_b, int D, int j, int F,
+                                int L, int Kc, int* idx_out, double* score_out, double* all_scores) {
+  int L_eff = L > 1 ? L : 1;
+  int lo = F, hi = j - L_eff; /* candidates c in [lo, hi) */
+  int n = hi > lo ? hi - lo : 0;
+  int* ci = (int*)malloc(sizeof(int) * (size_t)(n > 0 ? n : 1));
+  double* cs = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  if (n_rows <= 0) { free(ci); free(cs); return -1; }
+  if (all_scores)
+    for (int c = 0; c < n_b; ++c) all_scores[c] = NAN;
+  for (int c = 0; c < n; ++c) {
+    ci[c] = lo + c;
+    cs[c] = max_dot(q_rows, n_rows, S_c + (size_t)(lo + c) * D, D);
+    if (all_scores) all_scores[lo + c] = cs[c];
+  }
+  for (int s = 0; s < Kc; ++s) {
+    idx_out[s] = -1;
+    if (score_out) score_out[s] = 0.0;
+  }
+  int cnt = topk_select(ci, cs, n, Kc, idx_out, score_out);
+  free(ci);
+  free(cs);
+  return cnt;
+}
+
+int hga_oracle_route_groups_max(const double* q_rows, int n_rows, const double* S_g, int D, int gpc,
+                                const int* chunk_idx, int n_chunks, int Kg, int* idx_out, double* score_out,
+                                double* cand_scores) {
+  int n = n_chunks * gpc;
+  int* ci = (int*)malloc(sizeof(int) * (size_t)(n > 0 ? n : 1));
+  double* cs = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  if (n_rows <= 0) { free(ci); free(cs); return -1; }
+  for (int a = 0; a < n_chunks; ++a)
+    for (int u = 0; u < gpc; ++u) {
+      int g = chunk_idx[a] * gpc + u;
+      ci[a * gpc + u] = g;
+      cs[a * gpc + u] = max_dot(q_rows, n_rows, S_g + (size_t)g * D, D);
+      if (cand_scores) cand_scores[a * gpc + u] = cs[a * gpc + u];
+    }
+  for (int s = 0; s < Kg; ++s) {
+    idx_out[s] = -1;
+    if (score_out) score_out[s] = 0.0;
+  }
+  int cnt = topk_select(ci, cs, n, Kg, idx_out, score_out);
+  free(ci);
+  free(cs);
+  return cnt;
+}
+
+/* ------------------------------------------------------------------------------------------------ */
 /* Union token set of block j (R13: set union):                                      */
 /*   sink chunks {0..min(F,j)-1}  U  local chunks {max(0,j-L_eff)..j-1}  U  tokens of the opened groups */
 /*   U  current chunk (the causal cut u <= t is applied per query row in O6).                          */
@@ -501,14 +571,26 @@ int hga_oracle_slice(const hga_oracle_params* p, const float* q_raw, const float
     /* O4, O5 */
     int* cidx = (int*)malloc(sizeof(int) * (size_t)(p->Kc > 0 ? p->Kc : 1));
     int* gidx = (int*)malloc(sizeof(int) * (size_t)(p->Kg > 0 ? p->Kg : 1));
-    int nc = hga_oracle_route_chunks(qbar, S_c, n_b, D, j, p->F, p->L, p->Kc, cidx,
-                                     chunk_score ? chunk_score + (size_t)bi * p->Kc : NULL,
-                                     chunk_all_scores ? chunk_all_scores + (size_t)bi * n_b : NULL);
+    int nc, ng;
     if (group_cand_scores)
       for (int s = 0; s < p->Kc * gpc; ++s) group_cand_scores[(size_t)bi * p->Kc * gpc + s] = NAN;
-    int ng = hga_oracle_route_groups(qbar, S_g, D, gpc, cidx, nc, p->Kg, gidx,
-                                     group_score ? group_score + (size_t)bi * p->Kg : NULL,
-                                     group_cand_scores ? group_cand_scores + (size_t)bi * p->Kc * gpc : NULL);
+    if (p->route_max) {
+      /* N3 / R19: per-query scores from the rotated queries as stored */
+      hga_oracle_round_io(q_blk, (size_t)G * C * D, p->io_bf16);
+      nc = hga_oracle_route_chunks_max(q_blk, G * C, S_c, n_b, D, j, p->F, p->L, p->Kc, cidx,
+                                       chunk_score ? chunk_score + (size_t)bi * p->Kc : NULL,
+                                       chunk_all_scores ? chunk_all_scores + (size_t)bi * n_b : NULL);
+      ng = hga_oracle_route_groups_max(q_blk, G * C, S_g, D, gpc, cidx, nc, p->Kg, gidx,
+                                       group_score ? group_score + (size_t)bi * p->Kg : NULL,
+                                       group_cand_scores ? group_cand_scores + (size_t)bi * p->Kc * gpc : NULL);
+    } else {
+      nc = hga_oracle_route_chunks(qbar, S_c, n_b, D, j, p->F, p->L, p->Kc, cidx,
+                                   chunk_score ? chunk_score + (size_t)bi * p->Kc : NULL,
+                                   chunk_all_scores ? chunk_all_scores + (size_t)bi * n_b : NULL);
+      ng = hga_oracle_route_groups(qbar, S_g, D, gpc, cidx, nc, p->Kg, gidx,
+                                   group_score ? group_score + (size_t)bi * p->Kg : NULL,
+                                   group_cand_scores ? group_cand_scores + (size_t)bi * p->Kc * gpc : NULL);
+    }
     if (chunk_idx) memcpy(chunk_idx + (size_t)bi * p->Kc, cidx, sizeof(int) * (size_t)p->Kc);
     if (group_idx) memcpy(group_idx + (size_t)bi * p->Kg, gidx, sizeof(int) * (size_t)p->Kg);
     if (n_chunks) n_chunks[bi] = nc;
@@ -592,8 +674,15 @@ int hga_oracle_step(const hga_oracle_params* p, const float* q_win, const float*
   if (q_pooled) memcpy(q_pooled, qbar, sizeof(double) * (size_t)D);
   {
     /* O4, O5 over the closed chunks */
-    int nc = hga_oracle_route_chunks(qbar, S_c, n_closed, D, j, p->F, p->L, p->Kc, cidx, chunk_score, NULL);
-    int ng = hga_oracle_route_groups(qbar, S_g, D, gpc, cidx, nc, p->Kg, gidx, group_score, NULL);
+    int nc, ng;
+    if (p->route_max) { /* N3 / R19 (with R17: the rows the step processes) */
+      hga_oracle_round_io(q_rot, (size_t)G * W * D, p->io_bf16);
+      nc = hga_oracle_route_chunks_max(q_rot, G * W, S_c, n_closed, D, j, p->F, p->L, p->Kc, cidx, chunk_score, NULL);
+      ng = hga_oracle_route_groups_max(q_rot, G * W, S_g, D, gpc, cidx, nc, p->Kg, gidx, group_score, NULL);
+    } else {
+      nc = hga_oracle_route_chunks(qbar, S_c, n_closed, D, j, p->F, p->L, p->Kc, cidx, chunk_score, NULL);
+      ng = hga_oracle_route_groups(qbar, S_g, D, gpc, cidx, nc, p->Kg, gidx, group_score, NULL);
+    }
     if (chunk_idx) memcpy(chunk_idx, cidx, sizeof(int) * (size_t)p->Kc);
     if (group_idx) memcpy(group_idx, gidx, sizeof(int) * (size_t)p->Kg);
     if (n_chunks) *n_chunks = nc;

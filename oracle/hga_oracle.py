@@ -34,6 +34,7 @@ class _Params(C.Structure):
         ("F", C.c_int32), ("L", C.c_int32), ("Kc", C.c_int32), ("Kg", C.c_int32),
         ("n_hi_chunk", C.c_int32), ("n_hi_group", C.c_int32), ("io_bf16", C.c_int32),
         ("pos0", C.c_int64), ("base", C.c_double), ("scale", C.c_double), ("pos_mod", C.c_int64),
+        ("route_max", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
@@ -55,18 +56,20 @@ class OracleParams:
     base: float = 1.0e4
     scale: float = 0.0
     pos_mod: int = 0  # N3: RoPE position index wrapped modulo pos_mod; 0 = off
+    route_max: bool = False  # N3 (R4's alternative, R19): block score = max over the 64*G per-query scores
 
     def c_struct(self) -> _Params:
         return _Params(self.G, self.N, self.D, self.C, self.gs, self.F, self.L, self.Kc, self.Kg,
                        self.n_hi_chunk, self.n_hi_group, int(self.io_bf16), self.pos0, self.base, self.scale,
-                       self.pos_mod)
+                       self.pos_mod, int(self.route_max), 0)
 
 
 def params_from_workload(w) -> OracleParams:
     return OracleParams(G=w.n_q_heads // w.n_kv_heads, N=w.seq, D=w.head_dim, C=w.chunk, gs=w.group, F=w.n_sink,
                         L=w.n_local, Kc=w.topk_chunks, Kg=w.topk_groups, io_bf16=(w.dtype == "bf16"),
                         pos0=w.pos0, base=w.rope_base, pos_mod=getattr(w, "rope_pos_mod", 0),
-                        n_hi_chunk=getattr(w, "n_hi_chunk", -1), n_hi_group=getattr(w, "n_hi_group", -1))
+                        n_hi_chunk=getattr(w, "n_hi_chunk", -1), n_hi_group=getattr(w, "n_hi_group", -1),
+                        route_max=bool(getattr(w, "route_max", False)))
 
 
 def _L():
@@ -182,6 +185,35 @@ def route_groups(qbar_j, S_g, gpc: int, chunk_idx: Sequence[int], Kg: int):
     cnt = _L().hga_oracle_route_groups(_p(qbar_j, C.c_double), _p(S_g, C.c_double), C.c_int(D), C.c_int(gpc),
                                        _p(ci, C.c_int), C.c_int(len(ci)), C.c_int(Kg), _p(idx, C.c_int),
                                        _p(sc, C.c_double), _p(cand, C.c_double))
+    return idx[:Kg], sc[:Kg], int(cnt), cand[:len(ci) * gpc]
+
+
+def route_chunks_max(q_rows, S_c, j: int, F: int, L: int, Kc: int):
+    """N3 (R4's alternative): score(c) = max over the rows of q_rows [n_rows, D] of q . S_c[c].  Returns as route_chunks."""
+    q_rows, S_c = _f64(q_rows), _f64(S_c)
+    n_b, D = S_c.shape
+    q_rows = np.ascontiguousarray(q_rows.reshape(-1, D))
+    idx = np.empty(max(Kc, 1), dtype=np.int32)
+    sc = np.empty(max(Kc, 1), dtype=np.float64)
+    alls = np.empty(n_b, dtype=np.float64)
+    cnt = _L().hga_oracle_route_chunks_max(_p(q_rows, C.c_double), C.c_int(q_rows.shape[0]), _p(S_c, C.c_double),
+                                           C.c_int(n_b), C.c_int(D), C.c_int(j), C.c_int(F), C.c_int(L), C.c_int(Kc),
+                                           _p(idx, C.c_int), _p(sc, C.c_double), _p(alls, C.c_double))
+    return idx[:Kc], sc[:Kc], int(cnt), alls
+
+
+def route_groups_max(q_rows, S_g, gpc: int, chunk_idx: Sequence[int], Kg: int):
+    """N3: score(g) = max over the rows of q_rows of q . S_g[g].  Returns as route_groups."""
+    q_rows, S_g = _f64(q_rows), _f64(S_g)
+    D = S_g.shape[1]
+    q_rows = np.ascontiguousarray(q_rows.reshape(-1, D))
+    ci = _i32([c for c in chunk_idx if c >= 0])
+    idx = np.empty(max(Kg, 1), dtype=np.int32)
+    sc = np.empty(max(Kg, 1), dtype=np.float64)
+    cand = np.empty(max(len(ci) * gpc, 1), dtype=np.float64)
+    cnt = _L().hga_oracle_route_groups_max(_p(q_rows, C.c_double), C.c_int(q_rows.shape[0]), _p(S_g, C.c_double),
+                                           C.c_int(D), C.c_int(gpc), _p(ci, C.c_int), C.c_int(len(ci)), C.c_int(Kg),
+                                           _p(idx, C.c_int), _p(sc, C.c_double), _p(cand, C.c_double))
     return idx[:Kg], sc[:Kg], int(cnt), cand[:len(ci) * gpc]
 
 

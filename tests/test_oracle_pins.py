@@ -2,6 +2,7 @@
 library routines (transformers' Qwen3 RoPE, torch SDPA, torch bf16 casts), closed forms, brute force, values the
 paper prints (tests/golden/paper_constants.txt) and invariants the method must have.  No GPU needed.
 """
+import dataclasses
 import math
 import os
 
@@ -638,3 +639,101 @@ def test_n_hi_rules_closed_form():
     assert [oracle.n_hi_rule(128, 1e6, s, r) for r in range(3) for s in (64, 16)] == [11, 5, 14, 8, 20, 13]
     with pytest.raises(ValueError):
         oracle.n_hi_rule(64, 1e4, 64, 3)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# N3: R4's alternative -- a block's score of a candidate is the MAX over its 64*G per-query scores (PAPER.md:33, 45,
+# 97 leave the reduction open; reading R19: per-query scores use the rotated queries as stored)
+# ---------------------------------------------------------------------------------------------------------------
+def _max_mode_inputs(seed, n_b=24, D=32, rows=48):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((rows, D)), rng.standard_normal((n_b, D)), rng.standard_normal((n_b * 4, D))
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_max_mode_equals_bruteforce_on_tiny_inputs(seed):
+    """score(c) = max_r q_r . S[c] written out with numpy, then a full lexsort (score desc, index asc) -- the
+    definition, not the oracle's routine; constructed exact ties included."""
+    q_rows, S_c, S_g = _max_mode_inputs(seed)
+    S_c[7] = S_c[5]   # exact ties between candidates
+    S_c[11] = S_c[5]
+    F, L, Kc, Kg, gpc = 1, 2, 6, 9, 4
+    for j in (0, 1, 3, 4, 9, 23):
+        idx, sc, cnt, alls = oracle.route_chunks_max(q_rows, S_c, j, F, L, Kc)
+        cand = np.arange(F, max(F, j - max(L, 1)))
+        full = (q_rows @ S_c.T).max(axis=0)
+        order = cand[np.lexsort((cand, -full[cand]))][:Kc]
+        assert cnt == len(order) and np.array_equal(idx[:cnt], np.sort(order)) and np.all(idx[cnt:] == -1)
+        assert np.allclose(alls[cand], full[cand], rtol=1e-13, atol=1e-13) and np.isnan(np.delete(alls, cand)).all()
+        if cnt:
+            gc = (np.sort(order)[:, None] * gpc + np.arange(gpc)[None]).reshape(-1)
+            gfull = (q_rows @ S_g.T).max(axis=0)
+            gorder = gc[np.lexsort((gc, -gfull[gc]))][:Kg]
+            gidx, gsc, gcnt, gcand = oracle.route_groups_max(q_rows, S_g, gpc, idx[:cnt], Kg)
+            assert gcnt == len(gorder) and np.array_equal(gidx[:gcnt], np.sort(gorder))
+            assert np.allclose(gcand, gfull[gc], rtol=1e-13, atol=1e-13)
+
+
+def test_max_mode_reduces_to_mean_mode_when_all_queries_are_equal_and_dominates_it():
+    q_rows, S_c, S_g = _max_mode_inputs(5)
+    one = np.repeat(q_rows[:1], 48, axis=0)
+    for j in (6, 15, 23):
+        a = oracle.route_chunks_max(one, S_c, j, 1, 1, 5)
+        b = oracle.route_chunks(one[0], S_c, j, 1, 1, 5)
+        assert np.array_equal(a[0], b[0]) and a[2] == b[2] and np.allclose(a[1], b[1], rtol=1e-14)
+        ga = oracle.route_groups_max(one, S_g, 4, a[0][:a[2]], 7)
+        gb = oracle.route_groups(one[0], S_g, 4, b[0][:b[2]], 7)
+        assert np.array_equal(ga[0], gb[0]) and np.allclose(ga[3], gb[3], rtol=1e-14)
+        # max over queries >= mean over queries = pooled-query score (P17 linearity), candidate by candidate
+        mx = oracle.route_chunks_max(q_rows, S_c, j, 1, 1, 5)[3]
+        mean = oracle.route_chunks(q_rows.mean(axis=0), S_c, j, 1, 1, 5)[3]
+        cand = ~np.isnan(mx)
+        assert np.array_equal(cand, ~np.isnan(mean)) and np.all(mx[cand] >= mean[cand] - 1e-12)
+
+
+def test_max_mode_invariances():
+    """Row order of the block does not matter; scaling every query by alpha > 0 keeps the sets; a single dominant query
+    decides the selection alone."""
+    q_rows, S_c, _ = _max_mode_inputs(9)
+    base = oracle.route_chunks_max(q_rows, S_c, 20, 1, 1, 6)
+    perm = np.random.default_rng(1).permutation(len(q_rows))
+    assert np.array_equal(oracle.route_chunks_max(q_rows[perm], S_c, 20, 1, 1, 6)[0], base[0])
+    assert np.array_equal(oracle.route_chunks_max(3.5 * q_rows, S_c, 20, 1, 1, 6)[0], base[0])
+    big = q_rows.copy()
+    big[17] = 100.0 * S_c[9]   # one query aligned with candidate 9: its score dwarfs every other
+    idx = oracle.route_chunks_max(big, S_c, 20, 1, 1, 1)[0]
+    assert idx[0] == 9
+    alone = oracle.route_chunks(big[17], S_c, 20, 1, 1, 6)[0]     # the mean rule applied to that single query
+    assert 9 in alone
+
+
+def test_max_mode_prefill_slice_causality_and_attention_on_its_own_sets():
+    """Whole-slice run with route_max: (a) index sets equal route_*_max applied to the stored rotated queries (R19);
+    (b) sets of earlier blocks ignore later tokens; (c) O6 is the exact softmax over the resulting union
+    set (same attention code as the mean rule, checked through dense_block on full coverage)."""
+    w = W.Workload("mx", 1, 1024, 4, 2, 64, "bf16", 1e4, topk_chunks=3, topk_groups=7, n_clusters=4)
+    q, k, v = W.generate(w, 3)
+    op = dataclasses.replace(oracle.params_from_workload(w), route_max=True)
+    r = oracle.prefill_slice(op, q[0, :2], k[0, 0], v[0, 0])
+    rm = oracle.prefill_slice(dataclasses.replace(op, route_max=False), q[0, :2], k[0, 0], v[0, 0])
+    assert not np.array_equal(r.chunk_idx, rm.chunk_idx)  # the two rules do differ on this input
+    for j in (5, 9, 15):
+        qb = oracle.round_io(oracle.rope(q[0, :2, j * 64:(j + 1) * 64], j * 64, w.rope_base), True)
+        idx, sc, cnt, alls = oracle.route_chunks_max(qb, r.chunk_sum, j, 1, 1, 3)
+        assert np.array_equal(idx, r.chunk_idx[j]) and cnt == r.n_chunks[j]
+        gidx = oracle.route_groups_max(qb, r.group_sum, 4, idx[:cnt], 7)[0]
+        assert np.array_equal(gidx, r.group_idx[j])
+        o, l, _ = oracle.attend_block(qb, r.k_rot, v[0, 0].astype(np.float64), j, 64, 16, 1, 1, r.group_idx[j])
+        assert np.abs(o - r.out[j]).max() < 1e-12
+    k2, q2 = k.copy(), q.copy()
+    k2[0, 0, 640:] += 1.0
+    q2[0, :2, 640:] -= 0.5
+    r2 = oracle.prefill_slice(op, q2[0, :2], k2[0, 0], v[0, 0])
+    assert np.array_equal(r2.chunk_idx[:10], r.chunk_idx[:10]) and np.array_equal(r2.group_idx[:10], r.group_idx[:10])
+    assert np.abs(r2.out[:10] - r.out[:10]).max() == 0.0
+    # full coverage under the max rule is still dense causal attention (Eq. (1), PAPER.md:281)
+    opd = dataclasses.replace(op, Kc=16, Kg=64)
+    rd = oracle.prefill_slice(opd, q[0, :2], k[0, 0], v[0, 0], blocks=[15])
+    qb = oracle.round_io(oracle.rope(q[0, :2, 960:1024], 960, w.rope_base), True)
+    ref, _ = oracle.dense_block(qb, rd.k_rot, v[0, 0].astype(np.float64), 15, 64)
+    assert np.abs(rd.out[0] - ref).max() < 1e-10
