@@ -471,6 +471,31 @@ def run_ours(args, w):
                  "what": "hga_prefill_window over the last chunk [N-64, N) and over the last token [N-1, N) of the "
                          "filled cache, all batch items and heads; CUDA events, mean of 20 calls (launch-bound)"}
 
+    # ---- N3 variant: the max-over-queries routing rule (exact fp64, slow), stage time only -------------------------
+    variants = None
+    if rank == 0 and w.dtype == "bf16":
+        try:
+            pm = p.replace(route_mode=hga.binding.ROUTE_MAX)
+            ws = torch.empty(hga.hga_workspace_bytes(pm), dtype=torch.uint8, device="cuda")
+            import ctypes as C
+
+            lib, cpm = hga.load_library(), pm.c()
+
+            def rmax():
+                rc = lib.hga_route_max(C.byref(cpm), buf.q_rot.data_ptr(), buf.chunk_sum.data_ptr(), buf.group_sum.data_ptr(),
+                                       buf.chunk_idx.data_ptr(), None, buf.n_chunks.data_ptr(), buf.group_idx.data_ptr(), None,
+                                       buf.n_groups.data_ptr(), ws.data_ptr(), ws.numel(), torch.cuda.current_stream().cuda_stream)
+                assert rc == 0
+
+            variants = {"route_max_ms": sep(rmax, reps=3),
+                        "what": "hga_route_max (N3: block score = max over the 64*G per-query scores, fp64 SIMT) on the same "
+                                "tensors; the default pooled-query rule is stages.S2S3_route"}
+            del ws
+            hga.hga_prefill(p, dq, dk, dv, buf)  # restore the default rule's lists in buf
+            torch.cuda.synchronize()
+        except Exception as e:  # a variant must never sink the headline line
+            variants = {"error": str(e)}
+
     # ---- the other headline length: c4 (32K) beside c5 (64K), same measurement, inside the same JSON line ---------
     other = None
     other_name = {"c5": "c4", "c4": "c5"}.get(w.name)
@@ -534,6 +559,7 @@ def run_ours(args, w):
         "stages": stages,
         "sustained": sustained,
         "streaming": streaming,
+        "variants": variants,
         "roofline_floor_ms": roofline_floor_ms,
         "frac_of_roofline_floor": roofline_floor_ms / ms_per_step,
     }

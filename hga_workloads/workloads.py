@@ -31,6 +31,7 @@ class Workload:
     cluster_scale: float = 2.0
     pos0: int = 0
     rope_pos_mod: int = 0  # N3: RoPE position index wrapped modulo this value; 0 = off
+    route_max: bool = False  # N3 (R19): block score = max over per-query scores, not the pooled query
     n_hi_chunk: int = -1  # leading high-frequency RoPE pairs at chunk / group level (R1); -1 = default rule
     n_hi_group: int = -1
     n_valid: int = 0  # prompt tokens actually present (ragged tail); 0 = seq.  `seq` is then the cache capacity

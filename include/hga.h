@@ -62,6 +62,9 @@ typedef enum {
 
 typedef enum { HGA_F32 = 0, HGA_BF16 = 1 } hga_dtype;
 
+/* How a query block scores a routing candidate (see hga_params). */
+typedef enum { HGA_ROUTE_MEAN = 0, HGA_ROUTE_MAX = 1 } hga_route_mode;
+
 /* Which S4 kernel hga_attend launches. */
 typedef enum {
   HGA_ATTEND_AUTO = 0,    /* bf16 -> tcgen05/TMEM kernel (HGA_ATTEND_TCGEN05), f32 -> SIMT fp32 kernel */
@@ -93,6 +96,11 @@ typedef enum {
  *   (Q, K, both summary rules) is wrapped modulo it; the routing algorithm is unchanged.  It and pos0 must then be
  *   multiples of `chunk`, so that no chunk or group straddles a wrap (its middle position is the wrapped start +
  *   (S-1)/2); otherwise HGA_ERR_INVALID_ARG.  0 = off.
+ *   route_mode (variant; PAPER.md:33, 45, 97 do not say how a block's 64*G queries become one routing score):
+ *   HGA_ROUTE_MEAN = dot product with the pooled query (= mean of the per-query scores), the default;
+ *   HGA_ROUTE_MAX = the maximum over the block's per-query scores, each the dot product of a rotated query AS STORED
+ *   (rounded to io_dtype) with the summary.  Exact (fp64) but slow: a (64*G) x candidates x head_dim contraction per
+ *   block on the fp64 pipe.  hga_prefill honours it; the stand-alone call is hga_route_max.  Whole query blocks only.
  */
 typedef struct hga_params {
   int32_t batch, seq, n_q_heads, n_kv_heads, head_dim;
@@ -107,6 +115,8 @@ typedef struct hga_params {
   double rope_base;
   float softmax_scale;
   int32_t rope_pos_mod; /* 0 = off */
+  int32_t route_mode;   /* hga_route_mode */
+  int32_t reserved_;    /* must be 0 */
 } hga_params;
 
 HGA_API const char* hga_status_string(hga_status s);
@@ -161,6 +171,17 @@ HGA_API hga_status hga_route(const hga_params* p, const float* q_pooled, const f
                              const float* group_sum, int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks,
                              int32_t* group_idx, float* group_score, int32_t* n_groups, void* workspace,
                              size_t workspace_bytes, void* stream);
+
+/*
+ * S2 + S3 under HGA_ROUTE_MAX (p->route_mode must be HGA_ROUTE_MAX): the same candidate sets, budgets, tie rule and
+ * outputs as hga_route, with score(candidate) = max over the 64*G rotated queries of block j (all heads of the GQA
+ * group, read from q_rot [B,H_q,N,D] in io_dtype) of <q, summary> in fp64.  hga_route itself rejects HGA_ROUTE_MAX
+ * (HGA_ERR_INVALID_ARG): it is given no per-query tensor.  workspace: hga_workspace_bytes(p) bytes (larger in this mode).
+ */
+HGA_API hga_status hga_route_max(const hga_params* p, const void* q_rot, const float* chunk_sum,
+                                 const float* group_sum, int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks,
+                                 int32_t* group_idx, float* group_score, int32_t* n_groups, void* workspace,
+                                 size_t workspace_bytes, void* stream);
 
 /*
  * S4.  For query row (b,h,t) in block j = t / chunk with kv = h / (n_q_heads/n_kv_heads):

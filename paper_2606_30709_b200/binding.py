@@ -13,6 +13,7 @@ _LIB_PATH = os.path.join(_PKG, "libhga.so")
 _lib = None
 
 HGA_F32, HGA_BF16 = 0, 1
+ROUTE_MEAN, ROUTE_MAX = 0, 1
 ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM, ATTEND_TCGEN05_PAIR = 0, 1, 2, 3, 4
 
 
@@ -30,6 +31,7 @@ class _CParams(C.Structure):
         ("n_local", C.c_int32), ("topk_chunks", C.c_int32), ("topk_groups", C.c_int32), ("n_hi_chunk", C.c_int32),
         ("n_hi_group", C.c_int32), ("io_dtype", C.c_int32), ("out_dtype", C.c_int32), ("attend_impl", C.c_int32),
         ("pos0", C.c_int64), ("rope_base", C.c_double), ("softmax_scale", C.c_float), ("rope_pos_mod", C.c_int32),
+        ("route_mode", C.c_int32), ("reserved_", C.c_int32),
     ]
 
 
@@ -65,6 +67,7 @@ def load_library():
     lib.hga_rope.argtypes = [P, V, I, V, F, V]
     lib.hga_build_summaries.argtypes = [P, V, V, F, F, V]
     lib.hga_route.argtypes = [P, F, F, F, V, F, V, V, F, V, V, C.c_size_t, V]
+    lib.hga_route_max.argtypes = [P, V, F, F, V, F, V, V, F, V, V, C.c_size_t, V]
     lib.hga_attend.argtypes = [P, V, V, V, V, V, F, V]
     lib.hga_prefill.argtypes = [P, C.POINTER(_CBuffers), V]
     lib.hga_prefill_window.argtypes = [P, C.POINTER(_CBuffers), C.c_int64, C.c_int64, V]
@@ -102,12 +105,13 @@ class Params:
     rope_base: float = 1.0e4
     softmax_scale: float = 0.0
     rope_pos_mod: int = 0
+    route_mode: int = 0  # ROUTE_MEAN / ROUTE_MAX
 
     def c(self) -> _CParams:
         return _CParams(self.batch, self.seq, self.n_q_heads, self.n_kv_heads, self.head_dim, self.chunk, self.group,
                         self.n_sink, self.n_local, self.topk_chunks, self.topk_groups, self.n_hi_chunk, self.n_hi_group,
                         self.io_dtype, self.out_dtype, self.attend_impl, self.pos0, self.rope_base, self.softmax_scale,
-                        self.rope_pos_mod)
+                        self.rope_pos_mod, self.route_mode, 0)
 
     @property
     def n_blocks(self) -> int:
@@ -131,7 +135,7 @@ def params_from_workload(w, out_dtype: int = HGA_F32, attend_impl: int = ATTEND_
                   topk_groups=w.topk_groups, io_dtype=HGA_BF16 if w.dtype == "bf16" else HGA_F32, out_dtype=out_dtype,
                   attend_impl=attend_impl, pos0=w.pos0, rope_base=w.rope_base,
                   n_hi_chunk=getattr(w, "n_hi_chunk", -1), n_hi_group=getattr(w, "n_hi_group", -1),
-                  rope_pos_mod=getattr(w, "rope_pos_mod", 0))
+                  rope_pos_mod=getattr(w, "rope_pos_mod", 0), route_mode=int(bool(getattr(w, "route_max", False))))
 
 
 def _check(code: int, what: str):

@@ -33,6 +33,8 @@ hga_status validate(const hga_params* p) {
   if (p->out_dtype != HGA_F32 && p->out_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
   if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05_PAIR) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod < 0) return HGA_ERR_INVALID_ARG;
+  if (p->route_mode != HGA_ROUTE_MEAN && p->route_mode != HGA_ROUTE_MAX) return HGA_ERR_INVALID_ARG;
+  if (p->reserved_ != 0) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod > 0 && (p->rope_pos_mod % p->chunk || p->pos0 % p->chunk)) return HGA_ERR_INVALID_ARG;
   if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
   // what the kernels implement
@@ -60,6 +62,7 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
   d->n_hi_g = p->n_hi_group >= 0 ? p->n_hi_group : default_n_hi(p->head_dim, p->rope_base, p->group);
   d->pos0 = p->pos0;
   d->pos_mod = p->rope_pos_mod;
+  d->route_max = p->route_mode == HGA_ROUTE_MAX ? 1 : 0;
   d->scale = p->softmax_scale > 0.0f ? p->softmax_scale : (float)(1.0 / sqrt((double)p->head_dim));
   d->bf16_io = p->io_dtype == HGA_BF16;
   d->bf16_out = p->out_dtype == HGA_BF16;
@@ -73,7 +76,12 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static size_t score_ws_bytes(const Derived& d) {
-  return (size_t)d.B * d.Hkv * d.n_b * d.n_b * sizeof(float);
+  size_t n = (size_t)d.B * d.Hkv * d.n_b * d.n_b;  // chunk-score matrix
+  if (d.route_max) {
+    const int kc_cap = d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b;
+    n += (size_t)d.B * d.Hkv * d.n_b * kc_cap * d.gpc;  // group-candidate scores of the max rule
+  }
+  return n * sizeof(float);
 }
 
 }  // namespace hga
@@ -154,9 +162,25 @@ hga_status hga_route(const hga_params* p, const float* q_pooled, const float* ch
   if (!q_pooled || !chunk_sum || !chunk_idx) return HGA_ERR_INVALID_ARG;
   if (d.Kg > 0 && (!group_sum || !group_idx)) return HGA_ERR_INVALID_ARG;
   if (!aligned16(q_pooled) || !aligned16(chunk_sum) || !aligned16(group_sum)) return HGA_ERR_INVALID_ARG;
+  if (d.route_max) return HGA_ERR_INVALID_ARG;  // per-query scores need q_rot: hga_route_max
   if (!workspace || !aligned16(workspace) || workspace_bytes < score_ws_bytes(d)) return HGA_ERR_WORKSPACE;
   return launch_route(d, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
                       n_groups, (float*)workspace, (cudaStream_t)stream);
+}
+
+hga_status hga_route_max(const hga_params* p, const void* q_rot, const float* chunk_sum, const float* group_sum,
+                         int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx, float* group_score,
+                         int32_t* n_groups, void* workspace, size_t workspace_bytes, void* stream) {
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  if (!d.route_max) return HGA_ERR_INVALID_ARG;
+  if (!q_rot || !chunk_sum || !chunk_idx || !n_chunks) return HGA_ERR_INVALID_ARG;
+  if (d.Kg > 0 && (!group_sum || !group_idx)) return HGA_ERR_INVALID_ARG;
+  if (!aligned16(q_rot) || !aligned16(chunk_sum) || !aligned16(group_sum)) return HGA_ERR_INVALID_ARG;
+  if (!workspace || !aligned16(workspace) || workspace_bytes < score_ws_bytes(d)) return HGA_ERR_WORKSPACE;
+  return launch_route_max(d, q_rot, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
+                          n_groups, (float*)workspace, (cudaStream_t)stream);
 }
 
 static hga_status attend_blocks(const Derived& d, int impl, const void* q_rot, const void* k_rot, const void* v,
@@ -241,8 +265,15 @@ static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* 
   st = launch_rope_summaries(d, f, b->q_raw, b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum, cs);
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[1], cs));
-  st = launch_route(d, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
-                    b->group_score, b->n_groups, (float*)b->workspace, cs);
+  if (d.route_max) {
+    if (t_begin % kChunk != 0 || t_end % kChunk != 0) return HGA_ERR_UNSUPPORTED;  // whole query blocks only
+    if (!b->n_chunks) return HGA_ERR_INVALID_ARG;
+    st = launch_route_max(d, b->q_rot, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
+                          b->group_score, b->n_groups, (float*)b->workspace, cs);
+  } else {
+    st = launch_route(d, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
+                      b->group_score, b->n_groups, (float*)b->workspace, cs);
+  }
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[2], cs));
   st = attend_dispatch(d, p->attend_impl, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, cs);

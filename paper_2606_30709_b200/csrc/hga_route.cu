@@ -102,6 +102,113 @@ __global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_p
   }
 }
 
+// ----------------------------------------------------------------------------------------------------------------
+// N3, R4's alternative (reading R19): score of a candidate = MAX over the block's 64*G rotated
+// queries AS STORED of <q, S[cand]>, fp64 accumulation, d ascending.  One CTA = one (slice, block j, tile of 64
+// candidates); it walks the G heads of the group, each a 64-row x 64-candidate x D contraction with the micro-tiling
+// of score_kernel, and folds the rows away with a running max.  Candidates are either the dense chunk range
+// [64 tc, 64 tc + 64) of chunk_sum (cand == nullptr) or rows of group_sum gathered through the kept chunks of the unit
+// (group g = chunk_idx[a] * gpc + u for candidate a * gpc + u).  Exact but slow (fp64 SIMT over 64*G rows): the
+// variant costs ~8 ms at c5 against 0.04 ms for the pooled-query rule.
+// ----------------------------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ float to_f32(T v);
+template <>
+__device__ __forceinline__ float to_f32<float>(float v) { return v; }
+template <>
+__device__ __forceinline__ float to_f32<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
+
+template <typename T>
+__global__ void __launch_bounds__(64) score_max_kernel(const T* __restrict__ q_rot, const float* __restrict__ table,
+                                                       const int32_t* __restrict__ chunk_idx, const int32_t* __restrict__ n_chunks,
+                                                       float* __restrict__ out, int N, int n_b, int n_rows_tab, int D, int G, int Hkv,
+                                                       int F, int L_eff, int jb, int Kc, int gpc, int out_stride, bool groups) {
+  const int j = jb + (int)blockIdx.x;  // block of this CTA
+  const int tc = blockIdx.y;                                          // candidate tile
+  const size_t slice = blockIdx.z;                                    // b * Hkv + kv
+  const size_t unit = slice * n_b + j;
+  const int c0 = tc * kTile;
+  int n_cand;  // candidates of this unit in candidate order
+  if (groups) {
+    n_cand = n_chunks[unit] * gpc;
+  } else {
+    n_cand = j - L_eff;  // dense chunk range [0, j - L_eff); entries below F are computed but never read
+  }
+  if (c0 >= n_cand) return;  // block-uniform
+  __shared__ __align__(16) double Qs[kSlab][kTile];
+  __shared__ __align__(16) double Ss[kSlab][kTile];
+  __shared__ double red[8][kTile];
+  const int tid = threadIdx.x, tx = tid % 8, ty = tid / 8;
+  // row of `table` this thread stages (candidate c0 + tid)
+  long long srow = -1;
+  if (c0 + tid < n_cand) {
+    if (groups) {
+      const int cand = c0 + tid;
+      srow = (long long)chunk_idx[unit * Kc + cand / gpc] * gpc + cand % gpc;
+    } else {
+      srow = c0 + tid;
+    }
+  }
+  const float* S = table + slice * (size_t)n_rows_tab * D;
+  const int b = (int)(slice / Hkv), kv = (int)(slice % Hkv);
+  double best[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) best[i] = -CUDART_INF;
+  for (int h = 0; h < G; ++h) {
+    const T* Q = q_rot + (((size_t)b * Hkv * G + (size_t)kv * G + h) * N + (size_t)j * kChunk) * D;
+    double acc[8][8];
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+#pragma unroll
+      for (int bb = 0; bb < 8; ++bb) acc[a][bb] = 0.0;
+    for (int k0 = 0; k0 < D; k0 += kSlab) {
+      __syncthreads();
+      {
+        const T* qp = Q + (size_t)tid * D + k0;
+        const float* sp = S + (size_t)(srow < 0 ? 0 : srow) * D + k0;
+#pragma unroll
+        for (int u = 0; u < kSlab; ++u) {
+          Qs[u][tid] = (double)to_f32<T>(qp[u]);
+          Ss[u][tid] = srow < 0 ? 0.0 : (double)sp[u];
+        }
+      }
+      __syncthreads();
+#pragma unroll 4
+      for (int k = 0; k < kSlab; ++k) {
+        double qa[8], sb[8];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const double2 qv = *reinterpret_cast<const double2*>(&Qs[k][16 * i + 2 * ty]);
+          const double2 sv = *reinterpret_cast<const double2*>(&Ss[k][16 * i + 2 * tx]);
+          qa[2 * i] = qv.x; qa[2 * i + 1] = qv.y;
+          sb[2 * i] = sv.x; sb[2 * i + 1] = sv.y;
+        }
+#pragma unroll
+        for (int a = 0; a < 8; ++a)
+#pragma unroll
+          for (int bb = 0; bb < 8; ++bb) acc[a][bb] = fma(qa[a], sb[bb], acc[a][bb]);  // d ascending: fixed order
+      }
+    }
+#pragma unroll
+    for (int bb = 0; bb < 8; ++bb)
+#pragma unroll
+      for (int a = 0; a < 8; ++a) best[bb] = fmax(best[bb], acc[a][bb]);
+  }
+  // fold the 8 row-threads of every candidate column
+#pragma unroll
+  for (int b2 = 0; b2 < 4; ++b2) {
+    red[ty][16 * b2 + 2 * tx] = best[2 * b2];
+    red[ty][16 * b2 + 2 * tx + 1] = best[2 * b2 + 1];
+  }
+  __syncthreads();
+  if (c0 + tid < n_cand) {
+    double m = red[0][tid];
+#pragma unroll
+    for (int r = 1; r < 8; ++r) m = fmax(m, red[r][tid]);
+    out[unit * (size_t)out_stride + c0 + tid] = (float)m;
+  }
+}
+
 // Mark the `take` best of work[0..n) by overwriting them with -inf.  Order: score descending, index ascending (R8).
 __device__ __forceinline__ void warp_topk_mark(float* work, int n, int take, int lane) {
   for (int r = 0; r < take; ++r) {
@@ -128,7 +235,10 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
                                                      float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
                                                      int32_t* __restrict__ group_idx, float* __restrict__ group_score,
                                                      int32_t* __restrict__ n_groups, int n_units, int jb, int nj, int n_b, int n_g, int gpc,
-                                                     int F, int L_eff, int Kc, int Kg, int kc_cap, int per_warp_floats) {
+                                                     int F, int L_eff, int Kc, int Kg, int kc_cap, int per_warp_floats,
+                                                     int phase, const float* __restrict__ gscores_in) {
+  // phase 0: chunk top-K_c, then group refinement with pooled-query scores; 1: chunks only; 2: groups only, from the
+  // chunk lists already in chunk_idx / n_chunks and the candidate scores in gscores_in [unit][kc_cap * gpc] (N3 max rule)
   extern __shared__ __align__(16) float smem_f[];
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
   const int widx = blockIdx.x * (blockDim.x / 32) + warp;
@@ -144,15 +254,20 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
   const float* row = scores + (size_t)unit * n_b;
   const int lo = F, hi = j - L_eff;
   const int n = hi > lo ? hi - lo : 0;
-  for (int c = lane; c < n; c += 32) work[c] = row[lo + c];
-  __syncwarp();
-  const int take = min(Kc, n);
-  if (take < n) warp_topk_mark(work, n, take, lane);
-  // ascending compaction of the marked candidates
   int cnt = 0;
   int32_t* cidx = chunk_idx + (size_t)unit * Kc;
   float* csc = chunk_score ? chunk_score + (size_t)unit * Kc : nullptr;
-  for (int c0 = 0; c0 < n; c0 += 32) {
+  if (phase == 2) {
+    cnt = n_chunks[unit];
+    for (int c = lane; c < cnt; c += 32) sel[c] = cidx[c];
+    __syncwarp();
+  }
+  if (phase != 2) for (int c = lane; c < n; c += 32) work[c] = row[lo + c];
+  __syncwarp();
+  const int take = min(Kc, n);
+  if (phase != 2 && take < n) warp_topk_mark(work, n, take, lane);
+  // ascending compaction of the marked candidates
+  for (int c0 = 0; phase != 2 && c0 < n; c0 += 32) {
     const int c = c0 + lane;
     const bool on = c < n && (take == n || work[c] == -CUDART_INF_F);
     const unsigned m = __ballot_sync(0xffffffffu, on);
@@ -164,25 +279,37 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
     }
     cnt += __popc(m);
   }
-  for (int s = cnt + lane; s < Kc; s += 32) {
-    cidx[s] = -1;
-    if (csc) csc[s] = 0.f;
+  if (phase != 2) {
+    for (int s = cnt + lane; s < Kc; s += 32) {
+      cidx[s] = -1;
+      if (csc) csc[s] = 0.f;
+    }
+    if (n_chunks && lane == 0) n_chunks[unit] = cnt;
   }
-  if (n_chunks && lane == 0) n_chunks[unit] = cnt;
   __syncwarp();
-  if (Kg <= 0) return;
+  if (Kg <= 0 || phase == 1) return;
 
   // group refinement: candidates in ascending group order (sel is ascending)
   const int n_gc = cnt * gpc;
   constexpr int VPL = D / 32;  // values per lane
   float qv[VPL];
-  {
+  if (phase != 2) {
     const float* qp = q_pooled + (size_t)unit * D + lane * VPL;
 #pragma unroll
     for (int u = 0; u < VPL; ++u) qv[u] = qp[u];
+  } else {
+#pragma unroll
+    for (int u = 0; u < VPL; ++u) qv[u] = 0.f;
   }
   const float* gbase = group_sum + slice * (size_t)n_g * D;
-  for (int cand = 0; cand < n_gc; ++cand) {
+  if (phase == 2) {
+    for (int cand = lane; cand < n_gc; cand += 32) {
+      const float v = gscores_in[unit * (size_t)(kc_cap * gpc) + cand];
+      gwork[cand] = v;
+      gval[cand] = v;
+    }
+  }
+  for (int cand = 0; phase != 2 && cand < n_gc; ++cand) {
     const int g = sel[cand / gpc] * gpc + cand % gpc;
     const float* gp = gbase + (size_t)g * D + lane * VPL;
     double s = 0.0;
@@ -454,7 +581,47 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
                                                                n_chunks, group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b,
-                                                               d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp);
+                                                               d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 0, nullptr);
+  return launch_status();
+}
+
+// N3 max rule: chunk scores (max over the block's stored rotated queries) -> top-K_c -> group candidate scores of the
+// kept chunks -> top-K_g.  score_ws: [B, Hkv, n_b, n_b] chunk scores followed by [B, Hkv, n_b, kc_cap * gpc] group scores.
+hga_status launch_route_max(const Derived& d, const void* q_rot, const float* chunk_sum, const float* group_sum,
+                            int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
+                            float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
+  const int n_units = d.B * d.Hkv * d.nj;
+  const int kc_cap = d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b;
+  float* gscores = score_ws + (size_t)d.B * d.Hkv * d.n_b * d.n_b;
+  const int per_warp = d.n_b + 2 * kc_cap * d.gpc + kc_cap;
+  int warps = 4;
+  while (warps > 1 && (size_t)warps * per_warp * sizeof(float) > 200 * 1024) warps >>= 1;
+  const size_t smem = (size_t)warps * per_warp * sizeof(float);
+  if (smem > 200 * 1024) return HGA_ERR_UNSUPPORTED;
+  auto sel = d.D == 128 ? select_generic_kernel<128> : select_generic_kernel<64>;
+  HGA_CUDA_OK(cudaFuncSetAttribute(sel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int ct = (d.n_b + kTile - 1) / kTile, gt = (kc_cap * d.gpc + kTile - 1) / kTile;
+  auto run_scores = [&](bool groups, const float* table, int n_rows_tab, float* out, int out_stride, int tiles) {
+    dim3 grid(d.nj, tiles, d.B * d.Hkv);
+    if (d.bf16_io)
+      score_max_kernel<__nv_bfloat16><<<grid, 64, 0, s>>>((const __nv_bfloat16*)q_rot, table, chunk_idx, n_chunks, out, d.N, d.n_b,
+                                                          n_rows_tab, d.D, d.G, d.Hkv, d.F, d.L_eff, d.jb, d.Kc, d.gpc, out_stride, groups);
+    else
+      score_max_kernel<float><<<grid, 64, 0, s>>>((const float*)q_rot, table, chunk_idx, n_chunks, out, d.N, d.n_b, n_rows_tab,
+                                                  d.D, d.G, d.Hkv, d.F, d.L_eff, d.jb, d.Kc, d.gpc, out_stride, groups);
+  };
+  run_scores(false, chunk_sum, d.n_b, score_ws, d.n_b, ct);
+  if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+  sel<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, nullptr, group_sum, chunk_idx, chunk_score, n_chunks,
+                                                              group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g,
+                                                              d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 1, nullptr);
+  if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+  if (d.Kg <= 0) return HGA_OK;
+  run_scores(true, group_sum, d.n_g, gscores, kc_cap * d.gpc, gt);
+  if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+  sel<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, nullptr, group_sum, chunk_idx, chunk_score, n_chunks,
+                                                              group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g,
+                                                              d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 2, gscores);
   return launch_status();
 }
 

@@ -359,3 +359,59 @@ def test_pair_kernel_rejects_other_shapes():
     with pytest.raises(hga.HgaError) as e:
         hga.hga_attend(p, x, kv, kv, torch.full((1, 2, 8, 4), -1, dtype=torch.int32, device="cuda"))
     assert e.value.code == 2
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# N3: R4's alternative, max over the block's per-query scores (reading R19) -- the whole path
+# with hga_params.route_mode = HGA_ROUTE_MAX against the oracle's route_max switch, every block
+# ---------------------------------------------------------------------------------------------------------------
+ROUTE_MAX = [
+    # name, B, N, Hq, Hkv, D, dtype, base, Kc, Kg, F, L
+    ("mx_d64_g2", 1, 2048, 4, 2, 64, "bf16", 1e4, 5, 11, 1, 1),
+    ("mx_d128_g8", 1, 2048, 16, 2, 128, "bf16", 1e6, 6, 24, 1, 1),
+    ("mx_d128_g3_f2l3", 2, 1536, 6, 2, 128, "bf16", 1e6, 5, 7, 2, 3),
+    ("mx_f32", 1, 1024, 4, 1, 64, "f32", 1e4, 4, 8, 1, 1),
+    ("mx_kc40", 1, 4096, 2, 2, 64, "bf16", 1e4, 40, 50, 1, 1),   # 160 group candidates: three candidate tiles
+]
+
+
+@pytest.mark.parametrize("cfg", ROUTE_MAX, ids=[c[0] for c in ROUTE_MAX])
+def test_route_max_mode_full_parity(cfg):
+    name, B, N, Hq, Hkv, D, dt, base, Kc, Kg, F, L = cfg
+    w = W.Workload(name, B, N, Hq, Hkv, D, dt, base, n_sink=F, n_local=L, topk_chunks=Kc, topk_groups=Kg, n_clusters=8,
+                   dist="iid" if dt == "f32" else "clustered", route_max=True)
+    q, k, v = W.generate(w, 31)
+    p, buf = parity.run_gpu(w, q, k, v)
+    assert p.route_mode == hga.binding.ROUTE_MAX
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks * B * Hkv)
+    # the rule is not a no-op: the pooled-query rule picks other sets on the same input
+    p0, buf0 = parity.run_gpu(dataclasses.replace(w, route_max=False), q, k, v)
+    assert not torch.equal(buf.chunk_idx, buf0.chunk_idx)
+    # stand-alone call == what hga_prefill did; hga_route refuses the mode
+    lib = hga.load_library()
+    import ctypes as C
+    cp = p.c()
+    ci, gi = torch.empty_like(buf.chunk_idx), torch.empty_like(buf.group_idx)
+    nc, ng = torch.empty_like(buf.n_chunks), torch.empty_like(buf.n_groups)
+    st = torch.cuda.current_stream().cuda_stream
+    rc = lib.hga_route_max(C.byref(cp), buf.q_rot.data_ptr(), buf.chunk_sum.data_ptr(), buf.group_sum.data_ptr(),
+                           ci.data_ptr(), None, nc.data_ptr(), gi.data_ptr(), None, ng.data_ptr(), buf.workspace.data_ptr(),
+                           buf.workspace.numel(), st)
+    torch.cuda.synchronize()
+    assert rc == 0 and torch.equal(ci, buf.chunk_idx) and torch.equal(gi, buf.group_idx) and torch.equal(ng, buf.n_groups)
+    rc = lib.hga_route(C.byref(cp), buf.q_pooled.data_ptr(), buf.chunk_sum.data_ptr(), buf.group_sum.data_ptr(),
+                       ci.data_ptr(), None, nc.data_ptr(), gi.data_ptr(), None, ng.data_ptr(), buf.workspace.data_ptr(),
+                       buf.workspace.numel(), st)
+    assert rc == 1
+
+
+def test_route_max_mode_c5_full_size_sampled():
+    """The max rule at BASELINE.json configs[4] (64K, Qwen3 head shape): sampled blocks of two slices against the oracle."""
+    w = dataclasses.replace(W.get("c5"), route_max=True)
+    q, k, v = W.generate(w, 0)
+    p, buf = parity.run_gpu(w, q, k, v)
+    blocks = _sample_blocks(w.n_blocks, 12, 4)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [(0, 0), (0, 3)], blocks)
+    parity.assert_report(rep, w, 2 * len(blocks))
+    assert torch.isfinite(buf.out).all()
