@@ -63,7 +63,7 @@ typedef enum {
 typedef enum { HGA_F32 = 0, HGA_BF16 = 1 } hga_dtype;
 
 /* How a query block scores a routing candidate (see hga_params). */
-typedef enum { HGA_ROUTE_MEAN = 0, HGA_ROUTE_MAX = 1 } hga_route_mode;
+typedef enum { HGA_ROUTE_MEAN = 0, HGA_ROUTE_MAX = 1, HGA_ROUTE_MAX_FP64 = 2 } hga_route_mode;
 
 /* Which S4 kernel hga_attend launches. */
 typedef enum {
@@ -99,8 +99,15 @@ typedef enum {
  *   route_mode (variant; PAPER.md:33, 45, 97 do not say how a block's 64*G queries become one routing score):
  *   HGA_ROUTE_MEAN = dot product with the pooled query (= mean of the per-query scores), the default;
  *   HGA_ROUTE_MAX = the maximum over the block's per-query scores, each the dot product of a rotated query AS STORED
- *   (rounded to io_dtype) with the summary.  Exact (fp64) but slow: a (64*G) x candidates x head_dim contraction per
- *   block on the fp64 pipe.  hga_prefill honours it; the stand-alone call is hga_route_max.  Whole query blocks only.
+ *   (rounded to io_dtype) with the summary, in fp64 (d ascending, one fma chain).  hga_prefill honours it; the
+ *   stand-alone call is hga_route_max.  Whole query blocks only.
+ *   HGA_ROUTE_MAX_FP64 = the same rule with every (query, candidate) pair scored on the fp64 pipe: a (64*G) x candidates
+ *   x head_dim contraction per block (c5: 29 ms).  HGA_ROUTE_MAX returns the same lists and scores bit for bit, faster
+ *   (c5: 1.7 ms): for bf16 I/O, head_dim 64/128, G <= 8, K_c <= 64 and more than 128 blocks, a bf16 hi/lo tcgen05
+ *   contraction scores every pair approximately with a proven error bound, and only the candidates that can still reach
+ *   the top-K_c -- and, for each of them, only the query rows that can still hold the maximum -- are re-scored in fp64
+ *   (a unit whose near-ties exceed the 128-entry candidate list falls back to the fp64 contraction).  Other shapes run
+ *   the fp64 contraction under either value.
  */
 typedef struct hga_params {
   int32_t batch, seq, n_q_heads, n_kv_heads, head_dim;
@@ -173,7 +180,7 @@ HGA_API hga_status hga_route(const hga_params* p, const float* q_pooled, const f
                              size_t workspace_bytes, void* stream);
 
 /*
- * S2 + S3 under HGA_ROUTE_MAX (p->route_mode must be HGA_ROUTE_MAX): the same candidate sets, budgets, tie rule and
+ * S2 + S3 under HGA_ROUTE_MAX / HGA_ROUTE_MAX_FP64 (p->route_mode must be one of them): the same candidate sets, budgets, tie rule and
  * outputs as hga_route, with score(candidate) = max over the 64*G rotated queries of block j (all heads of the GQA
  * group, read from q_rot [B,H_q,N,D] in io_dtype) of <q, summary> in fp64.  hga_route itself rejects HGA_ROUTE_MAX
  * (HGA_ERR_INVALID_ARG): it is given no per-query tensor.  workspace: hga_workspace_bytes(p) bytes (larger in this mode).

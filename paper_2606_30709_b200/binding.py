@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_PKG, "libhga.so")
 _lib = None
 
 HGA_F32, HGA_BF16 = 0, 1
-ROUTE_MEAN, ROUTE_MAX = 0, 1
+ROUTE_MEAN, ROUTE_MAX, ROUTE_MAX_FP64 = 0, 1, 2
 ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM, ATTEND_TCGEN05_PAIR = 0, 1, 2, 3, 4
 
 
@@ -135,7 +135,7 @@ def params_from_workload(w, out_dtype: int = HGA_F32, attend_impl: int = ATTEND_
                   topk_groups=w.topk_groups, io_dtype=HGA_BF16 if w.dtype == "bf16" else HGA_F32, out_dtype=out_dtype,
                   attend_impl=attend_impl, pos0=w.pos0, rope_base=w.rope_base,
                   n_hi_chunk=getattr(w, "n_hi_chunk", -1), n_hi_group=getattr(w, "n_hi_group", -1),
-                  rope_pos_mod=getattr(w, "rope_pos_mod", 0), route_mode=int(bool(getattr(w, "route_max", False))))
+                  rope_pos_mod=getattr(w, "rope_pos_mod", 0), route_mode=int(getattr(w, "route_max", False)))
 
 
 def _check(code: int, what: str):

@@ -33,7 +33,8 @@ hga_status validate(const hga_params* p) {
   if (p->out_dtype != HGA_F32 && p->out_dtype != HGA_BF16) return HGA_ERR_INVALID_ARG;
   if (p->attend_impl < HGA_ATTEND_AUTO || p->attend_impl > HGA_ATTEND_TCGEN05_PAIR) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod < 0) return HGA_ERR_INVALID_ARG;
-  if (p->route_mode != HGA_ROUTE_MEAN && p->route_mode != HGA_ROUTE_MAX) return HGA_ERR_INVALID_ARG;
+  if (p->route_mode != HGA_ROUTE_MEAN && p->route_mode != HGA_ROUTE_MAX && p->route_mode != HGA_ROUTE_MAX_FP64)
+    return HGA_ERR_INVALID_ARG;
   if (p->reserved_ != 0) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod > 0 && (p->rope_pos_mod % p->chunk || p->pos0 % p->chunk)) return HGA_ERR_INVALID_ARG;
   if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
@@ -62,7 +63,7 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
   d->n_hi_g = p->n_hi_group >= 0 ? p->n_hi_group : default_n_hi(p->head_dim, p->rope_base, p->group);
   d->pos0 = p->pos0;
   d->pos_mod = p->rope_pos_mod;
-  d->route_max = p->route_mode == HGA_ROUTE_MAX ? 1 : 0;
+  d->route_max = p->route_mode;  // 0 mean, 1 max (tensor-core prefilter where eligible), 2 max on the fp64 pipe only
   d->scale = p->softmax_scale > 0.0f ? p->softmax_scale : (float)(1.0 / sqrt((double)p->head_dim));
   d->bf16_io = p->io_dtype == HGA_BF16;
   d->bf16_out = p->out_dtype == HGA_BF16;
@@ -76,12 +77,8 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static size_t score_ws_bytes(const Derived& d) {
-  size_t n = (size_t)d.B * d.Hkv * d.n_b * d.n_b;  // chunk-score matrix
-  if (d.route_max) {
-    const int kc_cap = d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b;
-    n += (size_t)d.B * d.Hkv * d.n_b * kc_cap * d.gpc;  // group-candidate scores of the max rule
-  }
-  return n * sizeof(float);
+  if (d.route_max) return route_max_ws_bytes(d);  // + group-candidate scores and the tensor-core prefilter's tables
+  return (size_t)d.B * d.Hkv * d.n_b * d.n_b * sizeof(float);  // chunk-score matrix
 }
 
 }  // namespace hga

@@ -30,6 +30,7 @@ struct Derived {
   long long pos_mod;  // RoPE position wrap; 0 = off
   float scale;              // softmax scale
   int route_max;            // N3: block score = max over per-query scores (R19) instead of the pooled-query score
+                            // (the hga_route_mode value: 1 = tensor-core prefilter where eligible, 2 = fp64 pipe only)
   bool bf16_io, bf16_out;
 };
 
@@ -99,6 +100,7 @@ hga_status launch_rope_summaries(const Derived& d, const RopeFreq& f, const void
 hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
                         int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s);
+size_t route_max_ws_bytes(const Derived& d);
 hga_status launch_route_max(const Derived& d, const void* q_rot, const float* chunk_sum, const float* group_sum,
                             int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                             float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s);

@@ -9,7 +9,10 @@
 //                  C/g_s groups of every kept chunk are scored (warp-cooperative fp64 dot products) and the top-K_g kept.
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "hga_common.cuh"
+#include "hga_tc_ptx.cuh"
 
 namespace hga {
 
@@ -122,11 +125,13 @@ template <typename T>
 __global__ void __launch_bounds__(64) score_max_kernel(const T* __restrict__ q_rot, const float* __restrict__ table,
                                                        const int32_t* __restrict__ chunk_idx, const int32_t* __restrict__ n_chunks,
                                                        float* __restrict__ out, int N, int n_b, int n_rows_tab, int D, int G, int Hkv,
-                                                       int F, int L_eff, int jb, int Kc, int gpc, int out_stride, bool groups) {
+                                                       int F, int L_eff, int jb, int Kc, int gpc, int out_stride, bool groups,
+                                                       const int32_t* __restrict__ only_neg) {
   const int j = jb + (int)blockIdx.x;  // block of this CTA
   const int tc = blockIdx.y;                                          // candidate tile
   const size_t slice = blockIdx.z;                                    // b * Hkv + kv
   const size_t unit = slice * n_b + j;
+  if (only_neg != nullptr && only_neg[unit] >= 0) return;  // block-uniform: only the flagged units are recomputed
   const int c0 = tc * kTile;
   int n_cand;  // candidates of this unit in candidate order
   if (groups) {
@@ -236,7 +241,8 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
                                                      int32_t* __restrict__ group_idx, float* __restrict__ group_score,
                                                      int32_t* __restrict__ n_groups, int n_units, int jb, int nj, int n_b, int n_g, int gpc,
                                                      int F, int L_eff, int Kc, int Kg, int kc_cap, int per_warp_floats,
-                                                     int phase, const float* __restrict__ gscores_in) {
+                                                     int phase, const float* __restrict__ gscores_in,
+                                                     const int32_t* __restrict__ only_neg) {
   // phase 0: chunk top-K_c, then group refinement with pooled-query scores; 1: chunks only; 2: groups only, from the
   // chunk lists already in chunk_idx / n_chunks and the candidate scores in gscores_in [unit][kc_cap * gpc] (N3 max rule)
   extern __shared__ __align__(16) float smem_f[];
@@ -251,6 +257,7 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
   const int j = jb + widx % nj;          // blocks [jb, jb + nj) of every slice
   const size_t slice = widx / nj;        // b * Hkv + kv
   const size_t unit = slice * n_b + j;   // row of every [B, Hkv, n_b, ...] table
+  if (only_neg != nullptr && only_neg[unit] >= 0) return;  // warp-uniform
   const float* row = scores + (size_t)unit * n_b;
   const int lo = F, hi = j - L_eff;
   const int n = hi > lo ? hi - lo : 0;
@@ -581,48 +588,712 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
                                                                n_chunks, group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b,
-                                                               d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 0, nullptr);
+                                                               d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 0, nullptr, nullptr);
   return launch_status();
 }
 
+}  // namespace hga (reopened below)
+
+namespace hga {
+
+namespace {
+
+// ----------------------------------------------------------------------------------------------------------------
+// N3 max rule on the tensor cores: approximate scores by a bf16 tcgen05 contraction, exact fp64 re-scoring of every
+// candidate that can still belong to the top-K_c.
+//   1. split_kernel        : S_c = hi + lo (two bf16 tables, |S_c - hi - lo| <= 2^-18 |S_c|) and |S_c|_2 per row;
+//   2. score_max_tc_kernel : per (slice, block j): D[cand, row] = sum_d S_c[cand, d] q[row, d] for 128 candidates x the
+//                            block's 64*G stored (bf16, exact) rotated queries, fp32 accumulation in TMEM, both bf16
+//                            parts of S_c; the epilogue folds the rows with a max -> approximate score s~(j, cand);
+//                            also q_max(j) = max_row |q_row|_2;
+//   3. band_kernel         : tau = K_c-th largest s~ of the unit; every candidate whose s~ is within the error bound of
+//                            tau (s~_c >= tau - E_max - e_c, e_c = eps |S_c|_2 q_max, eps = 2^-13 -- eight times the
+//                            worst case of the two-part split plus fp32 accumulation over 2D products) is listed: the
+//                            list provably contains the exact top-K_c;
+//   4. score_max_kernel    : exact fp64 scores of the listed candidates (gathered mode); 5. the generic selection
+//                            kernel's second phase picks the top-K_c of the list (ties -> lower index).
+// A unit whose band does not fit the list (more than kBandCap candidates within the bound: degenerate, tied inputs) is
+// flagged and recomputed by the dense fp64 path.
+// ----------------------------------------------------------------------------------------------------------------
+constexpr int kBandCap = 128;
+constexpr float kBandEps = 1.0f / 8192.0f;  // 2^-13
+
+template <int D>
+__global__ void __launch_bounds__(128) split_kernel(const float* __restrict__ table, __nv_bfloat16* __restrict__ hi,
+                                                    __nv_bfloat16* __restrict__ lo, float* __restrict__ norm, long long rows) {
+  const long long row = (long long)blockIdx.x * 4 + threadIdx.x / 32;
+  const int lane = threadIdx.x % 32;
+  if (row >= rows) return;
+  float ss = 0.f;
+  for (int d = lane; d < D; d += 32) {
+    const float v = table[row * D + d];
+    const __nv_bfloat16 h = __float2bfloat16_rn(v);
+    const __nv_bfloat16 l = __float2bfloat16_rn(v - __bfloat162float(h));
+    hi[row * D + d] = h;
+    lo[row * D + d] = l;
+    ss = fmaf(v, v, ss);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
+  if (lane == 0) norm[row] = sqrtf(ss) * (1.0f + 1e-6f);  // rounded up: it enters an upper bound
+}
+
+template <int D>
+struct TcS {
+  static constexpr int kHalves = D / 64;
+  static constexpr int kAHalf = 128 * 128;             // 128 candidates x 128 B
+  static constexpr int kAPart = kHalves * kAHalf;      // one bf16 part (hi or lo) of the candidate tile
+  static constexpr int kBHalf = 256 * 128;             // 256 query rows x 128 B
+  static constexpr int kBBlk = kHalves * kBHalf;       // one block of up to 256 query rows
+  static constexpr int kA = 0;
+  static constexpr int kB = 2 * kAPart;
+  static constexpr int kPairFlush = 128 * 32;          // (candidate, row) pairs one 32-column sweep can flag
+  static constexpr int kPairCap = 2 * kPairFlush;      // the list is emptied once it holds more than kPairFlush
+  // after the Q blocks: 3 mbarriers + the TMEM pointer (64 B), then the listed kernel's extras
+  __host__ __device__ static constexpr int bars_off(int nblk) { return kB + nblk * kBBlk; }
+  __host__ __device__ static constexpr int smem_bytes(int nblk) { return bars_off(nblk) + 64; }
+  static constexpr int kExtra = 128 * 8 + 128 * 4 + 128 * 4 + 16 + kPairCap * 2;  // best keys, e_c, table rows, counter, pairs
+  __host__ __device__ static constexpr int smem_bytes_listed(int nblk) { return smem_bytes(nblk) + kExtra; }
+};
+
+// Shared prologue of the two tensor-core kernels (all 128 threads): barriers, 512 TMEM columns, the block's queries
+// (G heads x 64 rows, 4 heads per 256-row block) by TMA; returns the TMEM base once the queries are in shared memory.
+template <int D>
+__device__ __forceinline__ uint32_t tc_load_queries(unsigned char* smem, const CUtensorMap* tmQ, int G, long long qrow0, int N,
+                                                    bool wait = true) {
+  using namespace tc;
+  using L = TcS<D>;
+  const uint32_t sbase = smem_u32(smem);
+  const int nblk = (G + 3) / 4;
+  const uint32_t bars = sbase + (uint32_t)L::bars_off(nblk);  // [0] Q loaded, [1] A loaded, [2] MMAs done
+  volatile uint32_t* tmem_p = reinterpret_cast<volatile uint32_t*>(smem + L::bars_off(nblk) + 32);
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  if (threadIdx.x == 0) {
+    if (sbase & 1023u) __trap();
+    mbar_init(bars + 0, 1);
+    mbar_init(bars + 8, 1);
+    mbar_init(bars + 16, 1);
+    fence_barrier_init();
+    fence_proxy_async();
+  }
+  if (warp == 0) tmem_alloc(sbase + (uint32_t)(L::bars_off(nblk) + 32), 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_p;
+  if (warp == 0) {
+    if (lane == 0) mbar_expect_tx(bars + 0, (uint32_t)(64 * G * D * 2));
+    __syncwarp();
+    for (int i = lane; i < G * L::kHalves; i += 32) {
+      const int h = i / L::kHalves, half = i % L::kHalves;
+      tma_load_2d(sbase + (uint32_t)(L::kB + (h / 4) * L::kBBlk + half * L::kBHalf + (h % 4) * 64 * 128), tmQ, half * 64,
+                  (int)(qrow0 + (long long)h * N), bars + 0);
+    }
+  }
+  if (wait) mbar_wait(bars + 0, 0);  // otherwise the caller waits on barrier 0 (parity 0) before it reads the queries
+  return tmem;
+}
+
+// max over the block's 64 G query rows of |q|_2, rounded up (it enters an error bound).  Eight lanes per row, one 16-byte
+// piece each (a quarter-warp reads one whole 128-byte row: no bank conflicts); the swizzle permutes the pieces of a row,
+// it does not mix rows.  Contains a __syncthreads.
+template <int D>
+__device__ __forceinline__ float tc_query_max_norm(const unsigned char* smem, int R, float* s_red) {
+  using L = TcS<D>;
+  float best = 0.f;
+  const int sub = threadIdx.x % 8;
+#pragma unroll 4
+  for (int r = threadIdx.x / 8; r < R; r += 16) {
+    float ss = 0.f;
+#pragma unroll
+    for (int half = 0; half < L::kHalves; ++half) {
+      const uint4 v = *reinterpret_cast<const uint4*>(smem + L::kB + (r / 256) * L::kBBlk + half * L::kBHalf + (r % 256) * 128 + sub * 16);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float a0 = __uint_as_float(w[u] << 16), a1 = __uint_as_float(w[u] & 0xFFFF0000u);
+        ss = fmaf(a0, a0, fmaf(a1, a1, ss));
+      }
+    }
+    ss += __shfl_xor_sync(0xffffffffu, ss, 1);
+    ss += __shfl_xor_sync(0xffffffffu, ss, 2);
+    ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+    best = fmaxf(best, ss);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) best = fmaxf(best, __shfl_xor_sync(0xffffffffu, best, off));
+  if (threadIdx.x % 32 == 0) s_red[threadIdx.x / 32] = best;
+  __syncthreads();
+  return sqrtf(fmaxf(fmaxf(s_red[0], s_red[1]), fmaxf(s_red[2], s_red[3]))) * (1.0f + 1e-5f);
+}
+
+// Warp 0, all lanes: D[cand, row] (TMEM, 128 lanes x 64 G columns) = (hi + lo)[cand, :] . q[row, :] for the candidate tile
+// in shared memory; both bf16 parts accumulate into the same fp32 columns.  Commits to bars + 16.
+template <int D>
+__device__ __forceinline__ void tc_issue_tile(uint32_t sbase, uint32_t tmem, int G, uint32_t ld) {
+  using namespace tc;
+  using L = TcS<D>;
+  constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);  // SBO 1024 B, version 1, SWIZZLE_128B
+  constexpr uint32_t kLbo = (16u >> 4) << 16;
+  const int nblk = (G + 3) / 4;
+  for (int blk = 0; blk < nblk; ++blk) {
+    const int nrows = 64 * min(4, G - 4 * blk);
+    const uint32_t idesc = umma_idesc(128, nrows, false);
+    const uint32_t d = tmem + (uint32_t)(blk * 256);
+    const uint32_t bb = ((sbase + (uint32_t)(L::kB + blk * L::kBBlk)) & 0x3FFFFu) >> 4;
+#pragma unroll
+    for (int part = 0; part < 2; ++part) {
+      const uint32_t ab = ((sbase + (uint32_t)(L::kA + part * L::kAPart)) & 0x3FFFFu) >> 4;
+#pragma unroll
+      for (int kk = 0; kk < D / 16; ++kk) {
+        const uint32_t oa = (uint32_t)((kk / 4) * L::kAHalf + (kk % 4) * 32) >> 4;
+        const uint32_t ob = (uint32_t)((kk / 4) * L::kBHalf + (kk % 4) * 32) >> 4;
+        umma_ss_e(d, make_desc(ab + oa + kLbo, kDescHi), make_desc(bb + ob + kLbo, kDescHi), idesc, (part | kk) ? 1u : 0u, ld);
+      }
+    }
+  }
+  umma_commit_e(sbase + (uint32_t)L::bars_off(nblk) + 16, ld);
+}
+
+// This lane's (= candidate's) maximum over the block's query rows of the accumulator tile.
+__device__ __forceinline__ float tc_row_max(uint32_t taddr, int G) {
+  using namespace tc;
+  float best = -CUDART_INF_F;
+  const int nblk = (G + 3) / 4;
+  for (int blk = 0; blk < nblk; ++blk) {
+    const int nrows = 64 * min(4, G - 4 * blk);
+    for (int c0 = 0; c0 < nrows; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld32(taddr + (uint32_t)(blk * 256 + c0), v);
+      tmem_wait_ld();
+      float m0 = __uint_as_float(v[0]), m1 = __uint_as_float(v[1]);
+#pragma unroll
+      for (int c = 2; c < 32; c += 2) {
+        m0 = fmaxf(m0, __uint_as_float(v[c]));
+        m1 = fmaxf(m1, __uint_as_float(v[c + 1]));
+      }
+      best = fmaxf(best, fmaxf(m0, m1));
+    }
+  }
+  return best;
+}
+
+template <int D>
+__global__ void __launch_bounds__(128, 1)
+score_max_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmHi,
+                    const __grid_constant__ CUtensorMap tmLo, float* __restrict__ scores, float* __restrict__ qmax, int N, int n_b,
+                    int G, int Hkv, int F, int L_eff, int jb) {
+  using namespace tc;
+  using L = TcS<D>;
+  extern __shared__ __align__(1024) unsigned char smem[];
+  __shared__ float s_red[4];
+  const uint32_t sbase = smem_u32(smem);
+  const int j = jb + (int)blockIdx.x;
+  const size_t slice = blockIdx.y;
+  const size_t unit = slice * n_b + j;
+  const int n_cand = j - L_eff;
+  if (n_cand - F <= kBandCap) return;  // block-uniform: band_kernel lists every candidate of such a unit
+  const int nblk = (G + 3) / 4;
+  const uint32_t bars = sbase + (uint32_t)L::bars_off(nblk);
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const int b = (int)(slice / Hkv), kv = (int)(slice % Hkv);
+  const uint32_t ld = elect_one();  // meaningful in warp 0 only
+  const uint32_t tmem = tc_load_queries<D>(smem, &tmQ, G, ((long long)b * Hkv * G + (long long)kv * G) * N + (long long)j * kChunk, N);
+  {
+    const float qm = tc_query_max_norm<D>(smem, 64 * G, s_red);
+    if (threadIdx.x == 0) qmax[unit] = qm;
+  }
+  // ---- candidate tiles ---------------------------------------------------------------------------------------------------
+  const int n_tiles = (n_cand + 127) / 128;
+  const long long srow0 = (long long)slice * n_b;
+  auto load_tile = [&](int a) {  // warp 0, all lanes: both bf16 parts of candidates [128 a, 128 a + 128)
+    if (lane == 0) mbar_expect_tx(bars + 8, (uint32_t)(2 * L::kAPart));
+    __syncwarp();
+    if (lane < 2 * L::kHalves) {
+      const int part = lane / L::kHalves, half = lane % L::kHalves;
+      tma_load_2d(sbase + (uint32_t)(L::kA + part * L::kAPart + half * L::kAHalf), part == 0 ? &tmHi : &tmLo, half * 64,
+                  (int)(srow0 + 128 * a), bars + 8);
+    }
+  };
+  if (warp == 0) load_tile(0);
+  for (int a = 0; a < n_tiles; ++a) {
+    if (warp == 0) {
+      mbar_wait(bars + 8, (uint32_t)a & 1u);
+      tc_fence_after();
+      tc_issue_tile<D>(sbase, tmem, G, ld);
+    }
+    mbar_wait(bars + 16, (uint32_t)a & 1u);
+    tc_fence_after();
+    if (warp == 0 && a + 1 < n_tiles) load_tile(a + 1);  // the MMAs have read the tile: the next one loads under the epilogue
+    const float best = tc_row_max(tmem + ((uint32_t)(warp * 32) << 16), G);
+    const int cand = 128 * a + warp * 32 + lane;
+    if (cand < n_b) scores[unit * (size_t)n_b + cand] = best;
+    tc_fence_before();
+    __syncthreads();  // every lane has read its accumulator row; the candidate tile and TMEM may be overwritten
+    tc_fence_after();
+  }
+  if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+// -DHGA_ROUTE_TRACE: cycles per phase of score_max_listed_kernel summed over its CTAs (hga_debug_route_trace)
+#ifdef HGA_ROUTE_TRACE
+__device__ unsigned long long g_rt[16];
+#define HGA_RT_BEGIN long long t0_ = clock64()
+#define HGA_RT(i)                                              \
+  do {                                                         \
+    if (threadIdx.x == 0) {                                    \
+      const long long t_ = clock64();                          \
+      atomicAdd(&g_rt[i], (unsigned long long)(t_ - t0_));     \
+      t0_ = t_;                                                \
+    }                                                          \
+  } while (0)
+#else
+#define HGA_RT_BEGIN do { } while (0)
+#define HGA_RT(i) do { } while (0)
+#endif
+
+__device__ __forceinline__ long long f64_key(double v) {  // order-preserving map of doubles onto signed integers
+  const long long b = __double_as_longlong(v);
+  return b >= 0 ? b : b ^ 0x7FFFFFFFFFFFFFFFll;
+}
+
+// Exact max-rule scores of LISTED candidates (the band of possible top-K_c chunks, or the group candidates of the kept
+// chunks): out[unit][i] = max over the block's 64 G stored queries of <q, table row of candidate i> in fp64 (d ascending,
+// one fma chain -- the same value score_max_kernel computes), found without scoring every (candidate, query) pair in
+// fp64: the bf16 hi/lo tensor-core contraction gives every pair's score a~ with |a~ - a| <= e_c (e_c = eps |S_c| q_max,
+// as in band_kernel); with m~ = max over queries of a~, the maximising query of the exact scores has a~ >= m~ - 2 e_c,
+// so only the pairs within 2 e_c of their candidate's m~ (usually one) are re-scored exactly.
+// Candidate i of a unit is table row  list[unit * list_stride + i / gpc] * gpc + i % gpc  (gpc = 1: the list holds rows).
+template <int D>
+__global__ void __launch_bounds__(128, 1)
+score_max_listed_kernel(const __grid_constant__ CUtensorMap tmQ, const float* __restrict__ table, const int32_t* __restrict__ list, const int32_t* __restrict__ cnt,
+                        float* __restrict__ out, int N, int n_b, int n_rows_tab, int G, int Hkv, int jb, int list_stride, int gpc,
+                        int out_stride) {
+  using namespace tc;
+  using L = TcS<D>;
+  extern __shared__ __align__(1024) unsigned char smem[];
+  __shared__ float s_red[4];
+  const uint32_t sbase = smem_u32(smem);
+  const int j = jb + (int)blockIdx.x;
+  const size_t slice = blockIdx.y;
+  const size_t unit = slice * n_b + j;
+  const int n_l = cnt[unit] * gpc;
+  if (n_l <= 0) return;  // block-uniform (also the units flagged -1 for the dense path)
+  const int nblk = (G + 3) / 4;
+  const int R = 64 * G;
+  const uint32_t bars = sbase + (uint32_t)L::bars_off(nblk);
+  unsigned char* extra = smem + L::smem_bytes(nblk);
+  long long* best_key = reinterpret_cast<long long*>(extra);          // [128]
+  float* s_norm = reinterpret_cast<float*>(extra + 128 * 8);          // [128] |S_c|_2 of the tile's candidates, rounded up
+  int* trow = reinterpret_cast<int*>(extra + 128 * 8 + 128 * 4);      // [128] table row of the tile's candidates
+  int* n_pairs = reinterpret_cast<int*>(extra + 128 * 8 + 128 * 8);   // pairs listed (degenerate path)
+  uint16_t* pairs = reinterpret_cast<uint16_t*>(extra + 128 * 8 + 128 * 8 + 16);  // [kPairCap] (candidate << 9) | row
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const int b = (int)(slice / Hkv), kv = (int)(slice % Hkv);
+  const uint32_t ld = elect_one();
+  HGA_RT_BEGIN;
+  // the queries load (TMA) under the staging of the first candidate tile
+  const uint32_t tmem = tc_load_queries<D>(smem, &tmQ, G, ((long long)b * Hkv * G + (long long)kv * G) * N + (long long)j * kChunk, N,
+                                           false);
+  HGA_RT(0);
+  const float* S = table + slice * (size_t)n_rows_tab * D;
+  const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16);
+  const int n_tiles = (n_l + 127) / 128;
+  const int me = warp * 32 + lane;  // this thread's candidate of a tile (its TMEM lane)
+  float qm = 0.f;
+  for (int a = 0; a < n_tiles; ++a) {
+    // ---- stage the tile: fp32 rows -> bf16 hi + lo in the swizzled K-major layout, one warp per row, eight rows in
+    // flight.  Dead rows keep whatever the tile held: their accumulator lanes are never read.
+    const int n_live = min(128, n_l - 128 * a);
+    {
+      const int ci = 128 * a + me;
+      trow[me] = me < n_live ? list[unit * list_stride + ci / gpc] * gpc + ci % gpc : -1;
+      best_key[me] = f64_key(-CUDART_INF);
+      if (me == 0) n_pairs[0] = 0;
+    }
+    __syncthreads();
+    for (int i0 = warp; i0 < n_live; i0 += 32) {
+      float4 v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int i = i0 + 4 * u;
+        v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i < n_live && 4 * lane < D) v[u] = *reinterpret_cast<const float4*>(S + (size_t)trow[i] * D + 4 * lane);
+      }
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int i = i0 + 4 * u;
+        if (i >= n_live) break;  // warp-uniform
+        if (4 * lane < D) {
+          const float f[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+          uint32_t h[2], l[2];
+#pragma unroll
+          for (int t = 0; t < 2; ++t) {
+            const __nv_bfloat16 h0 = __float2bfloat16_rn(f[2 * t]), h1 = __float2bfloat16_rn(f[2 * t + 1]);
+            const __nv_bfloat16 l0 = __float2bfloat16_rn(f[2 * t] - __bfloat162float(h0));
+            const __nv_bfloat16 l1 = __float2bfloat16_rn(f[2 * t + 1] - __bfloat162float(h1));
+            h[t] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+            l[t] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+          }
+          const int half = (4 * lane) / 64, piece = ((4 * lane) % 64) / 8;  // 16-byte piece of the 128-byte row
+          const int off = half * L::kAHalf + i * 128 + ((piece ^ (i % 8)) * 16) + (lane % 2) * 8;
+          *reinterpret_cast<uint2*>(smem + L::kA + off) = make_uint2(h[0], h[1]);
+          *reinterpret_cast<uint2*>(smem + L::kA + L::kAPart + off) = make_uint2(l[0], l[1]);
+        }
+        float ss = fmaf(v[u].x, v[u].x, fmaf(v[u].y, v[u].y, fmaf(v[u].z, v[u].z, v[u].w * v[u].w)));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        if (lane == 0) s_norm[i] = sqrtf(ss) * (1.0f + 1e-5f);
+      }
+    }
+    fence_proxy_async();  // the generic-proxy writes of the tile become visible to the tensor core
+    HGA_RT(1);
+    if (a == 0) {
+      mbar_wait(bars + 0, 0);  // the queries
+      qm = tc_query_max_norm<D>(smem, R, s_red);
+    } else {
+      __syncthreads();
+    }
+    HGA_RT(2);
+    if (warp == 0) {
+      tc_fence_after();
+      tc_issue_tile<D>(sbase, tmem, G, ld);
+    }
+    mbar_wait(bars + 16, (uint32_t)a & 1u);
+    tc_fence_after();
+    HGA_RT(3);
+    const bool live = me < n_live;
+    const float thr = tc_row_max(taddr, G) - 2.0f * kBandEps * qm * s_norm[me];
+    HGA_RT(4);
+    // ---- second sweep: the pairs within the bound, re-scored exactly -------------------------------------------------
+    // exact score of (candidate pc of the tile, query row r): fp64, d ascending, one fma chain
+    auto exact_pair = [&](int pc, int r) -> double {
+      const float* sp = S + (size_t)trow[pc] * D;
+      const unsigned char* qb = smem + L::kB + (r / 256) * L::kBBlk + (r % 256) * 128;
+      double acc = 0.0;
+#pragma unroll 8
+      for (int d0 = 0; d0 < D; d0 += 8) {
+        const uint4 qv = *reinterpret_cast<const uint4*>(qb + (d0 / 64) * L::kBHalf + ((((d0 % 64) / 8) ^ (r % 8)) * 16));
+        const float4 s0 = *reinterpret_cast<const float4*>(sp + d0), s1 = *reinterpret_cast<const float4*>(sp + d0 + 4);
+        const uint32_t w[4] = {qv.x, qv.y, qv.z, qv.w};
+        const float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          acc = fma((double)__uint_as_float(w[u] << 16), (double)sv[2 * u], acc);
+          acc = fma((double)__uint_as_float(w[u] & 0xFFFF0000u), (double)sv[2 * u + 1], acc);
+        }
+      }
+      return acc;
+    };
+    // bit mask of the columns [col0, col0 + 32) of this lane's accumulator row that reach thr
+    auto hits_of = [&](const uint32_t* v) -> uint32_t {
+      // most 32-column steps hold no pair of this lane: one max tree decides that
+      float m0 = max3(__uint_as_float(v[0]), __uint_as_float(v[1]), __uint_as_float(v[2]));
+      float m1 = max3(__uint_as_float(v[3]), __uint_as_float(v[4]), __uint_as_float(v[5]));
+#pragma unroll
+      for (int c = 6; c < 30; c += 4) {
+        m0 = max3(m0, __uint_as_float(v[c]), __uint_as_float(v[c + 1]));
+        m1 = max3(m1, __uint_as_float(v[c + 2]), __uint_as_float(v[c + 3]));
+      }
+      m0 = max3(m0, __uint_as_float(v[30]), __uint_as_float(v[31]));
+      uint32_t hit = 0;
+      if (live && fmaxf(m0, m1) >= thr) {
+        uint32_t h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+#pragma unroll
+        for (int c = 0; c < 32; c += 4) {
+          h0 |= (__uint_as_float(v[c]) >= thr ? 1u : 0u) << c;
+          h1 |= (__uint_as_float(v[c + 1]) >= thr ? 1u : 0u) << (c + 1);
+          h2 |= (__uint_as_float(v[c + 2]) >= thr ? 1u : 0u) << (c + 2);
+          h3 |= (__uint_as_float(v[c + 3]) >= thr ? 1u : 0u) << (c + 3);
+        }
+        hit = (h0 | h1) | (h2 | h3);
+      }
+      return hit;
+    };
+    // Usual case: at most four query rows per candidate are within the bound; every lane keeps its own rows in
+    // registers and re-scores them itself -- no list, no atomics, no barrier.
+    int hr0 = 0, hr1 = 0, hr2 = 0, hr3 = 0, nh = 0;
+    for (int blk = 0; blk < nblk; ++blk) {
+      const int nrows = 64 * min(4, G - 4 * blk);
+      for (int c0 = 0; c0 < nrows; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld32(taddr + (uint32_t)(blk * 256 + c0), v);
+        tmem_wait_ld();
+        uint32_t hit = hits_of(v);
+        while (hit) {
+          const int r = blk * 256 + c0 + __ffs(hit) - 1;
+          hit &= hit - 1;
+          if (nh == 0) hr0 = r;
+          else if (nh == 1) hr1 = r;
+          else if (nh == 2) hr2 = r;
+          else if (nh == 3) hr3 = r;
+          ++nh;
+        }
+      }
+    }
+    HGA_RT(5);
+    if (!__syncthreads_or(nh > 4)) {
+      if (live) {
+        double best = exact_pair(me, hr0);  // nh >= 1: the row of the approximate maximum is always within the bound
+        if (nh > 1) best = fmax(best, exact_pair(me, hr1));
+        if (nh > 2) best = fmax(best, exact_pair(me, hr2));
+        if (nh > 3) best = fmax(best, exact_pair(me, hr3));
+        out[unit * (size_t)out_stride + 128 * a + me] = (float)best;
+      }
+    } else {
+      // Degenerate inputs (many queries within the bound of the best, e.g. identical queries): (candidate, row) pairs go
+      // to a shared list that all threads empty together whenever one more 32-column step might not fit.
+      auto rescore = [&]() {  // all 128 threads; a barrier separates the list from the pushes
+        const int np = n_pairs[0];
+        for (int pi = threadIdx.x; pi < np; pi += 128) {
+          const int pc = pairs[pi] >> 9, r = pairs[pi] & 511;
+          atomicMax(&best_key[pc], f64_key(exact_pair(pc, r)));
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) n_pairs[0] = 0;
+        __syncthreads();
+      };
+      for (int blk = 0; blk < nblk; ++blk) {
+        const int nrows = 64 * min(4, G - 4 * blk);
+        for (int c0 = 0; c0 < nrows; c0 += 32) {
+          uint32_t v[32];
+          tmem_ld32(taddr + (uint32_t)(blk * 256 + c0), v);
+          tmem_wait_ld();
+          uint32_t hit = hits_of(v);
+          while (hit) {
+            const int c = __ffs(hit) - 1;
+            hit &= hit - 1;
+            pairs[atomicAdd(&n_pairs[0], 1)] = (uint16_t)((me << 9) | (blk * 256 + c0 + c));
+          }
+          if (__syncthreads_or(*reinterpret_cast<volatile int*>(&n_pairs[0]) > L::kPairFlush)) rescore();  // block-uniform
+        }
+      }
+      rescore();
+      if (live) {
+        const long long kb = best_key[me];
+        out[unit * (size_t)out_stride + 128 * a + me] = (float)__longlong_as_double(kb >= 0 ? kb : kb ^ 0x7FFFFFFFFFFFFFFFll);
+      }
+    }
+    HGA_RT(6);
+    tc_fence_before();
+    __syncthreads();  // the tile, its tables and TMEM are free for the next tile
+    tc_fence_after();
+  }
+  if (warp == 0) tmem_dealloc(tmem, 512);
+  HGA_RT(7);
+#ifdef HGA_ROUTE_TRACE
+  if (threadIdx.x == 0) atomicAdd(&g_rt[15], 1ull);
+#endif
+}
+
+// One warp per unit: the candidates whose approximate score can still reach the top-K_c (see the block comment above).
+__global__ void __launch_bounds__(128) band_kernel(const float* __restrict__ scores, const float* __restrict__ snorm,
+                                                   const float* __restrict__ qmax, int32_t* __restrict__ band_list,
+                                                   int32_t* __restrict__ band_cnt, int n_units, int jb, int nj, int n_b, int F,
+                                                   int L_eff, int Kc, int per_warp_floats) {
+  extern __shared__ __align__(16) float smem_f[];
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const int widx = blockIdx.x * (blockDim.x / 32) + warp;
+  if (widx >= n_units) return;
+  float* work = smem_f + (size_t)warp * per_warp_floats;  // [n_b]
+  const int j = jb + widx % nj;
+  const size_t slice = widx / nj;
+  const size_t unit = slice * n_b + j;
+  const float* row = scores + unit * (size_t)n_b;
+  const float* sn = snorm + slice * (size_t)n_b;
+  const int lo = F, hi = j - L_eff;
+  const int n = hi > lo ? hi - lo : 0;
+  int32_t* list = band_list + unit * (size_t)kBandCap;
+  if (n <= Kc || n <= kBandCap) {
+    // every candidate is kept (n <= K_c) or fits the list anyway: exact scores for all of them
+    const int m = min(n, kBandCap);
+    for (int c = lane; c < m; c += 32) list[c] = lo + c;
+    if (lane == 0) band_cnt[unit] = n <= kBandCap ? n : -1;
+    return;
+  }
+  float snmax = 0.f;
+  for (int c = lane; c < n; c += 32) {
+    work[c] = row[lo + c];
+    snmax = fmaxf(snmax, sn[lo + c]);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) snmax = fmaxf(snmax, __shfl_xor_sync(0xffffffffu, snmax, off));
+  __syncwarp();
+  warp_topk_mark(work, n, Kc, lane);  // the K_c best approximate scores become -inf in `work`
+  float tau = CUDART_INF_F;
+  for (int c = lane; c < n; c += 32)
+    if (work[c] == -CUDART_INF_F) tau = fminf(tau, row[lo + c]);
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) tau = fminf(tau, __shfl_xor_sync(0xffffffffu, tau, off));
+  const float qm = qmax[unit];
+  const float e_max = kBandEps * qm * snmax;
+  int cnt = 0;
+  bool overflow = false;
+  for (int c0 = 0; c0 < n; c0 += 32) {
+    const int c = c0 + lane;
+    const bool on = c < n && row[lo + c] >= tau - e_max - kBandEps * qm * sn[lo + c];
+    const unsigned mk = __ballot_sync(0xffffffffu, on);
+    const int pos = cnt + __popc(mk & ((1u << lane) - 1u));
+    if (on && pos < kBandCap) list[pos] = lo + c;
+    cnt += __popc(mk);
+  }
+  overflow = cnt > kBandCap;
+  if (lane == 0) band_cnt[unit] = overflow ? -1 : cnt;
+}
+
+}  // namespace
+
+// Workspace of the max rule, in floats: [B, Hkv, n_b, n_b] chunk scores | [B, Hkv, n_b, kc_cap * gpc] group-candidate
+// scores | (tensor-core path) S_hi, S_lo bf16 [rows, D] | |S_c| [rows] | q_max [units] | band_list int32 [units, kBandCap]
+// | band_cnt int32 [units] | band_score [units, kBandCap]; every part starts on a 256-byte boundary.
+namespace {
+struct MaxWs {
+  size_t gscores, s_hi, s_lo, snorm, qmax, band_list, band_cnt, band_score, total;  // offsets in floats
+};
+inline size_t up64(size_t n) { return (n + 63) & ~(size_t)63; }
+inline int max_kc_cap(const Derived& d) { return d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b; }
+inline MaxWs max_ws(const Derived& d) {
+  MaxWs w;
+  const size_t rows = (size_t)d.B * d.Hkv * d.n_b;
+  size_t o = up64(rows * d.n_b);
+  w.gscores = o; o += up64(rows * max_kc_cap(d) * d.gpc);
+  w.s_hi = o; o += up64(rows * d.D / 2);
+  w.s_lo = o; o += up64(rows * d.D / 2);
+  w.snorm = o; o += up64(rows);
+  w.qmax = o; o += up64(rows);
+  w.band_list = o; o += up64(rows * kBandCap);
+  w.band_cnt = o; o += up64(rows);
+  w.band_score = o; o += up64(rows * kBandCap);
+  w.total = o;
+  return w;
+}
+// the tensor-core path: bf16 queries (exact operands), D in {64, 128}, the block's 64 G query rows in 512 TMEM columns
+inline bool max_tc_eligible(const Derived& d) {
+  return d.route_max == 1 && d.bf16_io && (d.D == 64 || d.D == 128) && d.G <= 8 && d.Kc > 0 && d.Kc <= 64 && d.n_b > kBandCap;
+}
+}  // namespace
+
+size_t route_max_ws_bytes(const Derived& d) { return max_ws(d).total * sizeof(float); }
+
 // N3 max rule: chunk scores (max over the block's stored rotated queries) -> top-K_c -> group candidate scores of the
-// kept chunks -> top-K_g.  score_ws: [B, Hkv, n_b, n_b] chunk scores followed by [B, Hkv, n_b, kc_cap * gpc] group scores.
+// kept chunks -> top-K_g.
 hga_status launch_route_max(const Derived& d, const void* q_rot, const float* chunk_sum, const float* group_sum,
                             int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                             float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
   const int n_units = d.B * d.Hkv * d.nj;
-  const int kc_cap = d.Kc < d.n_b ? (d.Kc > 0 ? d.Kc : 1) : d.n_b;
-  float* gscores = score_ws + (size_t)d.B * d.Hkv * d.n_b * d.n_b;
-  const int per_warp = d.n_b + 2 * kc_cap * d.gpc + kc_cap;
+  const int kc_cap = max_kc_cap(d);
+  const MaxWs w = max_ws(d);
+  float* gscores = score_ws + w.gscores;
+  const bool use_tc = max_tc_eligible(d);
+  const int per_warp = d.n_b + 2 * (use_tc && kBandCap > kc_cap * d.gpc ? kBandCap : kc_cap * d.gpc) + (use_tc ? kBandCap : kc_cap);
   int warps = 4;
   while (warps > 1 && (size_t)warps * per_warp * sizeof(float) > 200 * 1024) warps >>= 1;
   const size_t smem = (size_t)warps * per_warp * sizeof(float);
   if (smem > 200 * 1024) return HGA_ERR_UNSUPPORTED;
   auto sel = d.D == 128 ? select_generic_kernel<128> : select_generic_kernel<64>;
   HGA_CUDA_OK(cudaFuncSetAttribute(sel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int sel_grid = (n_units + warps - 1) / warps;
   const int ct = (d.n_b + kTile - 1) / kTile, gt = (kc_cap * d.gpc + kTile - 1) / kTile;
-  auto run_scores = [&](bool groups, const float* table, int n_rows_tab, float* out, int out_stride, int tiles) {
+  // exact fp64 scores: dense over the chunk range (cidx == nullptr) or of the candidates listed in cidx / ncnt
+  auto run_scores = [&](bool listed, const float* table, int n_rows_tab, const int32_t* cidx, const int32_t* ncnt, int list_cap,
+                        int gpc, float* out, int out_stride, int tiles, const int32_t* only_neg) {
     dim3 grid(d.nj, tiles, d.B * d.Hkv);
     if (d.bf16_io)
-      score_max_kernel<__nv_bfloat16><<<grid, 64, 0, s>>>((const __nv_bfloat16*)q_rot, table, chunk_idx, n_chunks, out, d.N, d.n_b,
-                                                          n_rows_tab, d.D, d.G, d.Hkv, d.F, d.L_eff, d.jb, d.Kc, d.gpc, out_stride, groups);
+      score_max_kernel<__nv_bfloat16><<<grid, 64, 0, s>>>((const __nv_bfloat16*)q_rot, table, cidx, ncnt, out, d.N, d.n_b, n_rows_tab,
+                                                          d.D, d.G, d.Hkv, d.F, d.L_eff, d.jb, list_cap, gpc, out_stride, listed, only_neg);
     else
-      score_max_kernel<float><<<grid, 64, 0, s>>>((const float*)q_rot, table, chunk_idx, n_chunks, out, d.N, d.n_b, n_rows_tab,
-                                                  d.D, d.G, d.Hkv, d.F, d.L_eff, d.jb, d.Kc, d.gpc, out_stride, groups);
+      score_max_kernel<float><<<grid, 64, 0, s>>>((const float*)q_rot, table, cidx, ncnt, out, d.N, d.n_b, n_rows_tab, d.D, d.G,
+                                                  d.Hkv, d.F, d.L_eff, d.jb, list_cap, gpc, out_stride, listed, only_neg);
   };
-  run_scores(false, chunk_sum, d.n_b, score_ws, d.n_b, ct);
+  const int32_t* redo = nullptr;  // units the dense fp64 path still has to do (nullptr: all of them)
+  CUtensorMap tmQ;
+  // exact scores of listed candidates through the tensor-core row filter (score_max_listed_kernel)
+  auto run_listed = [&](const float* table, int n_rows_tab, const int32_t* cidx, const int32_t* ncnt, int list_stride, int gpc,
+                        float* out, int out_stride) -> bool {
+    const int nblk = (d.G + 3) / 4;
+    if (d.D == 128) {
+      const int sm = TcS<128>::smem_bytes_listed(nblk);
+      if (cudaFuncSetAttribute(score_max_listed_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return false;
+      score_max_listed_kernel<128><<<dim3(d.nj, d.B * d.Hkv), 128, sm, s>>>(tmQ, table, cidx, ncnt, out, d.N, d.n_b, n_rows_tab, d.G,
+                                                                           d.Hkv, d.jb, list_stride, gpc, out_stride);
+    } else {
+      const int sm = TcS<64>::smem_bytes_listed(nblk);
+      if (cudaFuncSetAttribute(score_max_listed_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return false;
+      score_max_listed_kernel<64><<<dim3(d.nj, d.B * d.Hkv), 128, sm, s>>>(tmQ, table, cidx, ncnt, out, d.N, d.n_b, n_rows_tab, d.G,
+                                                                          d.Hkv, d.jb, list_stride, gpc, out_stride);
+    }
+    return cudaGetLastError() == cudaSuccess;
+  };
+  if (use_tc) {
+    const long long rows = (long long)d.B * d.Hkv * d.n_b;
+    __nv_bfloat16* s_hi = reinterpret_cast<__nv_bfloat16*>(score_ws + w.s_hi);
+    __nv_bfloat16* s_lo = reinterpret_cast<__nv_bfloat16*>(score_ws + w.s_lo);
+    float* snorm = score_ws + w.snorm;
+    float* qmax = score_ws + w.qmax;
+    int32_t* band_list = reinterpret_cast<int32_t*>(score_ws + w.band_list);
+    int32_t* band_cnt = reinterpret_cast<int32_t*>(score_ws + w.band_cnt);
+    float* band_score = score_ws + w.band_score;
+    CUtensorMap tmHi, tmLo;
+    if (!tc::make_map_2d(&tmQ, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, q_rot, (uint64_t)d.B * d.Hq * d.N, d.D, 64, 64) ||
+        !tc::make_map_2d(&tmHi, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, s_hi, (uint64_t)rows, d.D, 64, 128) ||
+        !tc::make_map_2d(&tmLo, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, s_lo, (uint64_t)rows, d.D, 64, 128))
+      return HGA_ERR_CUDA;
+    const int nblk = (d.G + 3) / 4;
+    if (d.D == 128) {
+      split_kernel<128><<<(unsigned)((rows + 3) / 4), 128, 0, s>>>(chunk_sum, s_hi, s_lo, snorm, rows);
+      const int sm = TcS<128>::smem_bytes(nblk);
+      HGA_CUDA_OK(cudaFuncSetAttribute(score_max_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+      score_max_tc_kernel<128><<<dim3(d.nj, d.B * d.Hkv), 128, sm, s>>>(tmQ, tmHi, tmLo, score_ws, qmax, d.N, d.n_b, d.G, d.Hkv,
+                                                                       d.F, d.L_eff, d.jb);
+    } else {
+      split_kernel<64><<<(unsigned)((rows + 3) / 4), 128, 0, s>>>(chunk_sum, s_hi, s_lo, snorm, rows);
+      const int sm = TcS<64>::smem_bytes(nblk);
+      HGA_CUDA_OK(cudaFuncSetAttribute(score_max_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+      score_max_tc_kernel<64><<<dim3(d.nj, d.B * d.Hkv), 128, sm, s>>>(tmQ, tmHi, tmLo, score_ws, qmax, d.N, d.n_b, d.G, d.Hkv,
+                                                                      d.F, d.L_eff, d.jb);
+    }
+    if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+    {
+      int bw = 4;
+      while (bw > 1 && (size_t)bw * d.n_b * sizeof(float) > 200 * 1024) bw >>= 1;
+      const size_t bsm = (size_t)bw * d.n_b * sizeof(float);
+      if (bsm > 200 * 1024) return HGA_ERR_UNSUPPORTED;
+      HGA_CUDA_OK(cudaFuncSetAttribute(band_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsm));
+      band_kernel<<<(n_units + bw - 1) / bw, bw * 32, bsm, s>>>(score_ws, snorm, qmax, band_list, band_cnt, n_units, d.jb, d.nj,
+                                                               d.n_b, d.F, d.L_eff, d.Kc, d.n_b);
+    }
+    if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+    // exact scores of the listed candidates, then the top-K_c of each list ("groups" of one chunk each)
+    if (!run_listed(chunk_sum, d.n_b, band_list, band_cnt, kBandCap, 1, band_score, kBandCap)) return HGA_ERR_CUDA;
+    sel<<<sel_grid, warps * 32, smem, s>>>(score_ws, nullptr, chunk_sum, band_list, nullptr, band_cnt, chunk_idx, chunk_score,
+                                           n_chunks, n_units, d.jb, d.nj, d.n_b, d.n_b, 1, d.F, d.L_eff, kBandCap, d.Kc, kBandCap,
+                                           per_warp, 2, band_score, nullptr);
+    if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+    redo = band_cnt;  // units flagged -1: their band did not fit the list
+  }
+  run_scores(false, chunk_sum, d.n_b, nullptr, nullptr, d.Kc, d.gpc, score_ws, d.n_b, ct, redo);
   if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
-  sel<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, nullptr, group_sum, chunk_idx, chunk_score, n_chunks,
-                                                              group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g,
-                                                              d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 1, nullptr);
+  sel<<<sel_grid, warps * 32, smem, s>>>(score_ws, nullptr, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
+                                         n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap,
+                                         per_warp, 1, nullptr, redo);
   if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
   if (d.Kg <= 0) return HGA_OK;
-  run_scores(true, group_sum, d.n_g, gscores, kc_cap * d.gpc, gt);
-  if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
-  sel<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, nullptr, group_sum, chunk_idx, chunk_score, n_chunks,
-                                                              group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g,
-                                                              d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 2, gscores);
+  if (use_tc) {
+    if (!run_listed(group_sum, d.n_g, chunk_idx, n_chunks, d.Kc, d.gpc, gscores, kc_cap * d.gpc)) return HGA_ERR_CUDA;
+  } else {
+    run_scores(true, group_sum, d.n_g, chunk_idx, n_chunks, d.Kc, d.gpc, gscores, kc_cap * d.gpc, gt, nullptr);
+    if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
+  }
+  sel<<<sel_grid, warps * 32, smem, s>>>(score_ws, nullptr, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
+                                         n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap,
+                                         per_warp, 2, gscores, nullptr);
   return launch_status();
 }
 
 }  // namespace hga
+
+#ifdef HGA_ROUTE_TRACE
+extern "C" __attribute__((visibility("default"))) void hga_debug_route_trace(unsigned long long* out) {
+  cudaMemcpyFromSymbol(out, hga::g_rt, sizeof(unsigned long long) * 16);
+}
+#endif

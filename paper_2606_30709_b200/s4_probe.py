@@ -3,6 +3,8 @@ workload after one hga_prefill has produced the routed lists, and -- for a libra
 dumps the clock64 timeline of two work items of CTA 0 (softmax warpgroups and the MMA issuer).
 
     python -m paper_2606_30709_b200.s4_probe --workload c5 [--impl 2] [--lib path/to/libhga_variant.so] [--trace]
+    python -m paper_2606_30709_b200.s4_probe --workload c5 --route-max     (N3 max rule: both route modes timed and compared;
+                                                                            per-phase cycles with a -DHGA_ROUTE_TRACE build)
 
 Kernel experiments are compile-time knobs (HGA_S4_DIAG bit mask: 1 no softmax arithmetic, 2 no MMAs, 4 no MUFU,
 8 no K/V TMA; HGA_S4_EMU_PERIOD / _COUNT; HGA_S4_TRACE), set through HGA_NVCC_EXTRA:
@@ -17,6 +19,46 @@ import json
 import os
 
 
+def route_max_probe(B, w, dq, dk, dv, reps):
+    import torch
+
+    lib = B.load_library()
+    res = {}
+    for mode in (B.ROUTE_MAX, B.ROUTE_MAX_FP64):
+        p = B.params_from_workload(w).replace(route_mode=mode)
+        buf = B.hga_prefill(p, dq, dk, dv)
+        cp, st = p.c(), torch.cuda.current_stream().cuda_stream
+        nbytes = buf.workspace.numel() * buf.workspace.element_size()
+
+        def call():
+            rc = lib.hga_route_max(C.byref(cp), buf.q_rot.data_ptr(), buf.chunk_sum.data_ptr(), buf.group_sum.data_ptr(),
+                                   buf.chunk_idx.data_ptr(), buf.chunk_score.data_ptr(), buf.n_chunks.data_ptr(),
+                                   buf.group_idx.data_ptr(), buf.group_score.data_ptr(), buf.n_groups.data_ptr(),
+                                   buf.workspace.data_ptr(), nbytes, st)
+            assert rc == 0, rc
+
+        call()
+        torch.cuda.synchronize()
+        n = reps if mode == B.ROUTE_MAX else max(2, reps // 10)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            call()
+        e1.record()
+        torch.cuda.synchronize()
+        res[mode] = (e0.elapsed_time(e1) / n, [t.clone() for t in (buf.chunk_idx, buf.chunk_score, buf.n_chunks, buf.group_idx,
+                                                                   buf.group_score, buf.n_groups, buf.out)])
+    same = all(torch.equal(a, b) for a, b in zip(res[B.ROUTE_MAX][1], res[B.ROUTE_MAX_FP64][1]))
+    print(json.dumps({"workload": w.name, "route_max_ms": res[B.ROUTE_MAX][0], "route_max_fp64_ms": res[B.ROUTE_MAX_FP64][0],
+                      "bit_identical": same, "workspace_MB": nbytes / 1e6}))
+    if hasattr(lib, "hga_debug_route_trace"):
+        arr = (C.c_ulonglong * 16)()
+        lib.hga_debug_route_trace(arr)
+        n = max(int(arr[15]), 1)
+        names = ["setup + Q TMA issue", "stage candidate rows", "Q wait + q_max", "MMA", "row max", "sweep", "fp64 re-score", "dealloc"]
+        print("score_max_listed_kernel, CTAs", n, "| mean cycles per CTA:", {k: round(arr[i] / n) for i, k in enumerate(names)})
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--lib", default=None, help="alternative libhga.so (a build with experiment knobs)")
@@ -24,6 +66,7 @@ def main():
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--impl", type=int, default=0, help="hga_attend_impl (0 auto, 2 persistent, 4 CTA pair)")
     ap.add_argument("--trace", action="store_true", help="print the HGA_S4_TRACE timeline (needs a trace build)")
+    ap.add_argument("--route-max", action="store_true", help="time hga_route_max under HGA_ROUTE_MAX and HGA_ROUTE_MAX_FP64")
     args = ap.parse_args()
     import numpy as np
     import torch
@@ -37,6 +80,8 @@ def main():
     q, k, v = W.generate(w, 0)
     dt = torch.bfloat16 if w.dtype == "bf16" else torch.float32
     dq, dk, dv = (torch.from_numpy(a).to(dt).cuda() for a in (q, k, v))
+    if args.route_max:
+        return route_max_probe(B, w, dq, dk, dv, args.reps)
     p = B.params_from_workload(w, attend_impl=args.impl)
     buf = B.PrefillBuffers.allocate(p)
     for _ in range(3):

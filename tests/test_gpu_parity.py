@@ -406,6 +406,81 @@ def test_route_max_mode_full_parity(cfg):
     assert rc == 1
 
 
+# The tensor-core prefilter of the max rule (bf16, more than 128 blocks): approximate scores by a bf16 tcgen05 contraction,
+# exact fp64 re-scoring of every candidate within the error bound of the K_c-th best.  Against the oracle on sampled
+# blocks, and bit-identical to the fp64-only mode (HGA_ROUTE_MAX_FP64) on every block.
+ROUTE_MAX_TC = [
+    # name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L, dist
+    ("mxtc_d64_g2", 1, 16384, 4, 2, 64, 1e4, 5, 11, 1, 1, "clustered"),
+    ("mxtc_d128_g8", 1, 16384, 8, 1, 128, 1e6, 12, 48, 1, 1, "clustered"),
+    ("mxtc_d128_g3_f2l3", 2, 12288, 6, 2, 128, 1e6, 7, 9, 2, 3, "clustered"),
+    ("mxtc_d64_g6_iid", 1, 16384, 6, 1, 64, 1e4, 16, 64, 1, 1, "iid"),
+    ("mxtc_d128_g5_kc40", 1, 16384, 5, 1, 128, 1e4, 40, 50, 1, 2, "clustered"),
+    ("mxtc_d128_g1", 1, 24576, 2, 2, 128, 1e6, 8, 16, 1, 1, "iid"),
+]
+
+
+def _route_outputs(buf):
+    return [buf.chunk_idx, buf.chunk_score, buf.n_chunks, buf.group_idx, buf.group_score, buf.n_groups]
+
+
+@pytest.mark.parametrize("cfg", ROUTE_MAX_TC, ids=[c[0] for c in ROUTE_MAX_TC])
+def test_route_max_tensor_core_prefilter(cfg):
+    name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L, dist = cfg
+    w = W.Workload(name, B, N, Hq, Hkv, D, "bf16", base, n_sink=F, n_local=L, topk_chunks=Kc, topk_groups=Kg, n_clusters=8,
+                   dist=dist, route_max=True)
+    q, k, v = W.generate(w, 37)
+    p, buf = parity.run_gpu(w, q, k, v)
+    assert p.route_mode == hga.binding.ROUTE_MAX
+    p2, buf2 = parity.run_gpu(w, q, k, v, route_mode=hga.binding.ROUTE_MAX_FP64)
+    for a, b in zip(_route_outputs(buf), _route_outputs(buf2)):
+        assert torch.equal(a, b)
+    assert torch.equal(buf.out, buf2.out)
+    blocks = _sample_blocks(w.n_blocks, 10, 4)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [(B - 1, Hkv - 1)], blocks)
+    parity.assert_report(rep, w, len(blocks))
+
+
+def test_route_max_tensor_core_prefilter_ties_fall_back():
+    """Every chunk summary identical (keys periodic in the chunk length, RoPE positions wrapped at the chunk length): all
+    candidates tie exactly, the band of possible winners overflows its list and the unit is recomputed by the dense fp64
+    path -- the lowest indices win (R8), as in the fp64-only mode and the oracle."""
+    w = W.Workload("mxtc_ties", 1, 16384, 4, 2, 64, "bf16", 1e4, topk_chunks=6, topk_groups=12, n_clusters=8, route_max=True,
+                   rope_pos_mod=64)
+    q, k, v = W.generate(w, 5)
+    k = np.ascontiguousarray(np.tile(k[:, :, :64], (1, 1, w.n_blocks, 1)))
+    p, buf = parity.run_gpu(w, q, k, v)
+    p2, buf2 = parity.run_gpu(w, q, k, v, route_mode=hga.binding.ROUTE_MAX_FP64)
+    for a, b in zip(_route_outputs(buf), _route_outputs(buf2)):
+        assert torch.equal(a, b)
+    ci = buf.chunk_idx[0, 0].cpu().numpy()
+    j = w.n_blocks - 1
+    assert list(ci[j, :6]) == [1, 2, 3, 4, 5, 6]  # F = 1: candidates start at chunk 1; all tied -> lowest indices
+    blocks = _sample_blocks(w.n_blocks, 6, 2)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [(0, 1)], blocks)
+    parity.assert_report(rep, w, len(blocks))
+
+
+def test_route_max_tensor_core_prefilter_many_tied_queries():
+    """Blocks whose queries are all zero: every (candidate, query) pair scores exactly 0, so every query row is within the
+    error bound of the best and the exact re-scoring takes its list path (more than four rows per candidate); the other
+    blocks take the usual path.  Same result as the fp64-only mode and the oracle (all candidates tie -> lowest indices)."""
+    w = W.Workload("mxtc_zero_q", 1, 16384, 8, 1, 128, "bf16", 1e6, topk_chunks=6, topk_groups=12, n_clusters=8, route_max=True)
+    q, k, v = W.generate(w, 9)
+    zero_blocks = [3, 100, 101, 130, 200, 255]   # below and above the 128-candidate limit of the band list
+    for j in zero_blocks:
+        q[:, :, 64 * j:64 * (j + 1)] = 0.0
+    p, buf = parity.run_gpu(w, q, k, v)
+    p2, buf2 = parity.run_gpu(w, q, k, v, route_mode=hga.binding.ROUTE_MAX_FP64)
+    for a, b in zip(_route_outputs(buf), _route_outputs(buf2)):
+        assert torch.equal(a, b)
+    ci = buf.chunk_idx[0, 0].cpu().numpy()
+    assert list(ci[200, :6]) == [1, 2, 3, 4, 5, 6] and list(ci[100, :6]) == [1, 2, 3, 4, 5, 6]
+    blocks = np.array(sorted(set(zero_blocks) | {50, 150, 254}))
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [(0, 0)], blocks)
+    parity.assert_report(rep, w, len(blocks))
+
+
 def test_route_max_mode_c5_full_size_sampled():
     """The max rule at BASELINE.json configs[4] (64K, Qwen3 head shape): sampled blocks of two slices against the oracle."""
     w = dataclasses.replace(W.get("c5"), route_max=True)
