@@ -18,6 +18,24 @@ namespace hga {
 
 namespace {
 
+// -DHGA_ROUTE_TRACE: cycles per phase summed over the CTAs of score_max_listed_kernel (slots 0-7, count in 15) and over the
+// warps of select_fast_kernel (slots 16-23, count in 31); read back by hga_debug_route_trace
+#ifdef HGA_ROUTE_TRACE
+__device__ unsigned long long g_rt[32];
+#define HGA_RT_BEGIN long long t0_ = clock64()
+#define HGA_RT(i)                                                        \
+  do {                                                                   \
+    if (threadIdx.x % 32 == 0 && ((i) >= 16 || threadIdx.x == 0)) {      \
+      const long long t_ = clock64();                                    \
+      atomicAdd(&g_rt[i], (unsigned long long)(t_ - t0_));               \
+      t0_ = t_;                                                          \
+    }                                                                    \
+  } while (0)
+#else
+#define HGA_RT_BEGIN do { } while (0)
+#define HGA_RT(i) do { } while (0)
+#endif
+
 constexpr int kTile = 64;
 constexpr int kSlab = 32;
 
@@ -369,16 +387,23 @@ __device__ __forceinline__ uint32_t order_key(float v) {
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-// Best (value, offset) of the m candidates at `col`; ascending scan with strict '>' keeps the lowest offset.
+// Best (value, offset) of the m candidates at `col` (m a multiple of 4): the maximum by a max tree, then the lowest
+// offset that holds it (descending scan of independent equality tests: the last write is the lowest offset, R8).
 __device__ __forceinline__ void lane_rescan(const float* col, int m, float& bv, int& bo) {
-  bv = -CUDART_INF_F;
-  bo = 0;
+  float b0 = -CUDART_INF_F, b1 = -CUDART_INF_F;
   for (int o = 0; o < m; o += 4) {
     const float4 v = *reinterpret_cast<const float4*>(col + o);
-    if (v.x > bv) { bv = v.x; bo = o; }
-    if (v.y > bv) { bv = v.y; bo = o + 1; }
-    if (v.z > bv) { bv = v.z; bo = o + 2; }
-    if (v.w > bv) { bv = v.w; bo = o + 3; }
+    b0 = tc::max3(b0, v.x, v.y);
+    b1 = tc::max3(b1, v.z, v.w);
+  }
+  bv = fmaxf(b0, b1);
+  bo = 0;
+  for (int o = m - 4; o >= 0; o -= 4) {
+    const float4 v = *reinterpret_cast<const float4*>(col + o);
+    if (v.w == bv) bo = o + 3;
+    if (v.z == bv) bo = o + 2;
+    if (v.y == bv) bo = o + 1;
+    if (v.x == bv) bo = o;
   }
 }
 
@@ -396,8 +421,7 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
   if (widx >= n_units) return;  // warp-uniform; no block-wide barrier below
   const int m = 1 << lm, stride = m + 4;
   unsigned char* base = smem_sel + (size_t)warp * per_warp_bytes;
-  double* qd = reinterpret_cast<double*>(base);                 // [D]
-  float* work = reinterpret_cast<float*>(base + D * 8);         // [32][m + 4]
+  float* work = reinterpret_cast<float*>(base);                 // [32][m + 4]; after the chunk stage: the query as doubles [D]
   int* sel = reinterpret_cast<int*>(work + 32 * stride);        // [32]
 
   const int j = jb + widx % nj;          // blocks [jb, jb + nj) of every slice
@@ -408,8 +432,16 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
   const int n = hi > lo ? hi - lo : 0;
   int32_t* cidx = chunk_idx + (size_t)unit * Kc;
   float* csc = chunk_score ? chunk_score + (size_t)unit * Kc : nullptr;
+  // the pooled query of the unit, VPL consecutive values per lane (needed by the group stage: loaded early)
+  constexpr int VPL = D / 32;
+  float qf[VPL];
+  if (Kg > 0) {
+#pragma unroll
+    for (int u = 0; u < VPL; ++u) qf[u] = q_pooled[(size_t)unit * D + lane * VPL + u];
+  }
 
   // ---- stage the row (coalesced reads), pad with -inf -------------------------------------------------------
+  HGA_RT_BEGIN;
   const int n_lanes = (n + m - 1) >> lm;  // lanes that own at least one candidate
   for (int c = lane; c < n_lanes * m; c += 32) {
     const float v = c < n ? row[lo + c] : -CUDART_INF_F;
@@ -420,6 +452,7 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
   float bv = -CUDART_INF_F;
   int bo = 0;
   if (lane < n_lanes) lane_rescan(col, m, bv, bo);
+  HGA_RT(16);
 
   // ---- top-K_c: one winner per round, kept in lane r ---------------------------------------------------------
   const int take = min(Kc, n);
@@ -447,6 +480,7 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
       }
     }
   }
+  HGA_RT(17);
   // ---- ascending order: rank of this lane's winner among the winners ------------------------------------------
   int rank = 0;
 #pragma unroll
@@ -463,12 +497,19 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
   }
   if (n_chunks && lane == 0) n_chunks[unit] = cnt;
   if (Kg <= 0) return;
+  HGA_RT(18);
 
   // ---- group refinement: candidate `cand` = group cand % gpc of kept chunk cand / gpc (ascending group order) -----
+  // Scores: one candidate per lane, fp64 fma chain over d (ascending) with the pooled query in shared memory as doubles.
   const int n_gc = cnt * gpc;  // <= 128
-  {
-    const float* qp = q_pooled + (size_t)unit * D;
-    for (int d = lane; d < D; d += 32) qd[d] = (double)qp[d];
+  const int gtake = min(Kg, n_gc);
+  const bool need_scores = gtake < n_gc || group_score != nullptr;  // K_g >= candidates: every group is kept unscored
+  __syncwarp();  // sel[] complete; the candidate rows in `work` are no longer needed
+  HGA_RT(19);
+  double* qd = reinterpret_cast<double*>(work);  // [D] the pooled query as doubles (the candidate rows are no longer needed)
+  if (need_scores) {
+#pragma unroll
+    for (int u = 0; u < VPL; ++u) qd[lane * VPL + u] = (double)qf[u];
   }
   __syncwarp();
   const float* gbase = group_sum + slice * (size_t)n_g * D;
@@ -481,6 +522,9 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
     gid[i] = -1;
     if (cand < n_gc) {
       const int g = sel[cand / gpc] * gpc + cand % gpc;
+      gid[i] = g;
+      gsc[i] = 0.f;
+      if (!need_scores) continue;
       const float4* gp = reinterpret_cast<const float4*>(gbase + (size_t)g * D);
       double s = 0.0;
 #pragma unroll 4
@@ -497,7 +541,7 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
       gid[i] = g;
     }
   }
-  const int gtake = min(Kg, n_gc);
+  HGA_RT(20);
   unsigned taken = 0;  // bit i: candidate lane + 32*i is kept
   if (gtake == n_gc) {
 #pragma unroll
@@ -526,6 +570,7 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
       }
     }
   }
+  HGA_RT(21);
   // ascending compaction (candidates are in ascending group order)
   int gcnt = 0;
   int32_t* gidx = group_idx + (size_t)unit * Kg;
@@ -546,6 +591,10 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
     if (gscore) gscore[s] = 0.f;
   }
   if (n_groups && lane == 0) n_groups[unit] = gcnt;
+  HGA_RT(22);
+#ifdef HGA_ROUTE_TRACE
+  if (lane == 0) atomicAdd(&g_rt[31], 1ull);
+#endif
 }
 
 }  // namespace
@@ -565,7 +614,7 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
     const int n_max = d.n_b - d.F - d.L_eff > 1 ? d.n_b - d.F - d.L_eff : 1;
     int lm = 2;
     while ((32 << lm) < n_max) ++lm;
-    const int per_warp_bytes = d.D * 8 + 32 * ((1 << lm) + 4) * 4 + 32 * 4;
+    const int per_warp_bytes = 32 * ((1 << lm) + 4) * 4 + 32 * 4;
     int warps = 4;
     while (warps > 1 && (size_t)warps * per_warp_bytes > 200 * 1024) warps >>= 1;
     const size_t smem = (size_t)warps * per_warp_bytes;
@@ -834,23 +883,6 @@ score_max_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
   }
   if (warp == 0) tmem_dealloc(tmem, 512);
 }
-
-// -DHGA_ROUTE_TRACE: cycles per phase of score_max_listed_kernel summed over its CTAs (hga_debug_route_trace)
-#ifdef HGA_ROUTE_TRACE
-__device__ unsigned long long g_rt[16];
-#define HGA_RT_BEGIN long long t0_ = clock64()
-#define HGA_RT(i)                                              \
-  do {                                                         \
-    if (threadIdx.x == 0) {                                    \
-      const long long t_ = clock64();                          \
-      atomicAdd(&g_rt[i], (unsigned long long)(t_ - t0_));     \
-      t0_ = t_;                                                \
-    }                                                          \
-  } while (0)
-#else
-#define HGA_RT_BEGIN do { } while (0)
-#define HGA_RT(i) do { } while (0)
-#endif
 
 __device__ __forceinline__ long long f64_key(double v) {  // order-preserving map of doubles onto signed integers
   const long long b = __double_as_longlong(v);
@@ -1294,6 +1326,6 @@ hga_status launch_route_max(const Derived& d, const void* q_rot, const float* ch
 
 #ifdef HGA_ROUTE_TRACE
 extern "C" __attribute__((visibility("default"))) void hga_debug_route_trace(unsigned long long* out) {
-  cudaMemcpyFromSymbol(out, hga::g_rt, sizeof(unsigned long long) * 16);
+  cudaMemcpyFromSymbol(out, hga::g_rt, sizeof(unsigned long long) * 32);
 }
 #endif

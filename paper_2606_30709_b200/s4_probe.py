@@ -52,7 +52,7 @@ def route_max_probe(B, w, dq, dk, dv, reps):
     print(json.dumps({"workload": w.name, "route_max_ms": res[B.ROUTE_MAX][0], "route_max_fp64_ms": res[B.ROUTE_MAX_FP64][0],
                       "bit_identical": same, "workspace_MB": nbytes / 1e6}))
     if hasattr(lib, "hga_debug_route_trace"):
-        arr = (C.c_ulonglong * 16)()
+        arr = (C.c_ulonglong * 32)()
         lib.hga_debug_route_trace(arr)
         n = max(int(arr[15]), 1)
         names = ["setup + Q TMA issue", "stage candidate rows", "Q wait + q_max", "MMA", "row max", "sweep", "fp64 re-score", "dealloc"]
