@@ -65,6 +65,19 @@ typedef enum { HGA_F32 = 0, HGA_BF16 = 1 } hga_dtype;
 /* How a query block scores a routing candidate (see hga_params). */
 typedef enum { HGA_ROUTE_MEAN = 0, HGA_ROUTE_MAX = 1, HGA_ROUTE_MAX_FP64 = 2 } hga_route_mode;
 
+/* hga_params.flags */
+typedef enum {
+  /* N2: hga_prefill / hga_prefill_window / hga_host_prefill need not materialise the rotated
+   * queries.  S0 then only pools them (q_rot is not written and may be NULL), and S4 reads q_raw and applies RoPE
+   * to every query tile in shared memory, with the same fp32 arithmetic and the same single rounding to
+   * bf16 -- so 2 * |Q| bytes of HBM traffic (the Q_rot write and its read) disappear.  Conditions: io_dtype bf16, whole
+   * 64-token blocks, route_mode HGA_ROUTE_MEAN (the max rule reads q_rot), attend_impl HGA_ATTEND_AUTO or
+   * HGA_ATTEND_TCGEN05; anything else returns HGA_ERR_UNSUPPORTED (call again without the flag).  The (cos, sin) of a
+   * position is formed as the product of two table entries (block start x offset in the block), 2-3 ulp(fp32) instead of
+   * 1: a rotated query can differ from S0's by one bf16 rounding step in rare cases. */
+  HGA_FLAG_FUSE_Q_ROPE = 1
+} hga_flag;
+
 /* Which S4 kernel hga_attend launches. */
 typedef enum {
   HGA_ATTEND_AUTO = 0,    /* bf16 -> tcgen05/TMEM kernel (HGA_ATTEND_TCGEN05), f32 -> SIMT fp32 kernel */
@@ -123,7 +136,7 @@ typedef struct hga_params {
   float softmax_scale;
   int32_t rope_pos_mod; /* 0 = off */
   int32_t route_mode;   /* hga_route_mode */
-  int32_t reserved_;    /* must be 0 */
+  int32_t flags;        /* bit mask of hga_flag values; other bits must be 0 */
 } hga_params;
 
 HGA_API const char* hga_status_string(hga_status s);

@@ -14,6 +14,7 @@ _lib = None
 
 HGA_F32, HGA_BF16 = 0, 1
 ROUTE_MEAN, ROUTE_MAX, ROUTE_MAX_FP64 = 0, 1, 2
+FLAG_FUSE_Q_ROPE = 1
 ATTEND_AUTO, ATTEND_SIMT, ATTEND_TCGEN05, ATTEND_TCGEN05_ITEM, ATTEND_TCGEN05_PAIR = 0, 1, 2, 3, 4
 
 
@@ -31,7 +32,7 @@ class _CParams(C.Structure):
         ("n_local", C.c_int32), ("topk_chunks", C.c_int32), ("topk_groups", C.c_int32), ("n_hi_chunk", C.c_int32),
         ("n_hi_group", C.c_int32), ("io_dtype", C.c_int32), ("out_dtype", C.c_int32), ("attend_impl", C.c_int32),
         ("pos0", C.c_int64), ("rope_base", C.c_double), ("softmax_scale", C.c_float), ("rope_pos_mod", C.c_int32),
-        ("route_mode", C.c_int32), ("reserved_", C.c_int32),
+        ("route_mode", C.c_int32), ("flags", C.c_int32),
     ]
 
 
@@ -105,13 +106,14 @@ class Params:
     rope_base: float = 1.0e4
     softmax_scale: float = 0.0
     rope_pos_mod: int = 0
-    route_mode: int = 0  # ROUTE_MEAN / ROUTE_MAX
+    route_mode: int = 0  # ROUTE_MEAN / ROUTE_MAX / ROUTE_MAX_FP64
+    flags: int = 0       # FLAG_FUSE_Q_ROPE: q_rot is not materialised, S4 rotates its query tiles itself (N2)
 
     def c(self) -> _CParams:
         return _CParams(self.batch, self.seq, self.n_q_heads, self.n_kv_heads, self.head_dim, self.chunk, self.group,
                         self.n_sink, self.n_local, self.topk_chunks, self.topk_groups, self.n_hi_chunk, self.n_hi_group,
                         self.io_dtype, self.out_dtype, self.attend_impl, self.pos0, self.rope_base, self.softmax_scale,
-                        self.rope_pos_mod, self.route_mode, 0)
+                        self.rope_pos_mod, self.route_mode, self.flags)
 
     @property
     def n_blocks(self) -> int:
@@ -261,7 +263,7 @@ def hga_attend(p: Params, q_rot: torch.Tensor, k_rot: torch.Tensor, v: torch.Ten
 class PrefillBuffers:
     """Device buffers of one prefill pass (mirror of `hga_buffers`)."""
 
-    q_rot: torch.Tensor
+    q_rot: Optional[torch.Tensor]
     k_rot: torch.Tensor
     q_pooled: torch.Tensor
     chunk_sum: torch.Tensor
@@ -282,7 +284,8 @@ class PrefillBuffers:
         f32, i32 = torch.float32, torch.int32
         e = lambda shape, dt: torch.empty(shape, dtype=dt, device=device)
         return PrefillBuffers(
-            q_rot=e((p.batch, p.n_q_heads, p.seq, p.head_dim), p.torch_io),
+            # with FLAG_FUSE_Q_ROPE the rotated queries are never written: no buffer (a NULL pointer at the C boundary)
+            q_rot=None if p.flags & FLAG_FUSE_Q_ROPE else e((p.batch, p.n_q_heads, p.seq, p.head_dim), p.torch_io),
             k_rot=e((p.batch, p.n_kv_heads, p.seq, p.head_dim), p.torch_io),
             q_pooled=e(units + (p.head_dim,), f32), chunk_sum=e(units + (p.head_dim,), f32),
             group_sum=e((p.batch, p.n_kv_heads, p.seq // p.group, p.head_dim), f32),
@@ -301,7 +304,8 @@ def _cbuffers(q_raw, k_raw, v, buf, want_lse):
     cb.q_raw, cb.k_raw, cb.v = q_raw.data_ptr(), k_raw.data_ptr(), v.data_ptr()
     for name in ("q_rot", "k_rot", "q_pooled", "chunk_sum", "group_sum", "chunk_idx", "chunk_score", "n_chunks",
                  "group_idx", "group_score", "n_groups", "out", "workspace"):
-        setattr(cb, name, getattr(buf, name).data_ptr())
+        t = getattr(buf, name)
+        setattr(cb, name, t.data_ptr() if t is not None else None)
     cb.lse = buf.lse.data_ptr() if want_lse else None
     cb.workspace_bytes = buf.workspace.numel()
     return cb

@@ -35,7 +35,7 @@ hga_status validate(const hga_params* p) {
   if (p->rope_pos_mod < 0) return HGA_ERR_INVALID_ARG;
   if (p->route_mode != HGA_ROUTE_MEAN && p->route_mode != HGA_ROUTE_MAX && p->route_mode != HGA_ROUTE_MAX_FP64)
     return HGA_ERR_INVALID_ARG;
-  if (p->reserved_ != 0) return HGA_ERR_INVALID_ARG;
+  if (p->flags & ~(int32_t)HGA_FLAG_FUSE_Q_ROPE) return HGA_ERR_INVALID_ARG;
   if (p->rope_pos_mod > 0 && (p->rope_pos_mod % p->chunk || p->pos0 % p->chunk)) return HGA_ERR_INVALID_ARG;
   if (p->pos0 < 0 || p->pos0 + p->seq > (1ll << 40)) return HGA_ERR_INVALID_ARG;
   // what the kernels implement
@@ -64,6 +64,7 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
   d->pos0 = p->pos0;
   d->pos_mod = p->rope_pos_mod;
   d->route_max = p->route_mode;  // 0 mean, 1 max (tensor-core prefilter where eligible), 2 max on the fp64 pipe only
+  d->fuse_q_rope = (p->flags & HGA_FLAG_FUSE_Q_ROPE) ? 1 : 0;
   d->scale = p->softmax_scale > 0.0f ? p->softmax_scale : (float)(1.0 / sqrt((double)p->head_dim));
   d->bf16_io = p->io_dtype == HGA_BF16;
   d->bf16_out = p->out_dtype == HGA_BF16;
@@ -76,9 +77,19 @@ hga_status derive(const hga_params* p, Derived* d, RopeFreq* f) {
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// N2: the two RoPE tables of the fused S4 (launch_rope_tables) live behind the routing workspace
+static size_t rope_tables_bytes(const Derived& d) {
+  return d.fuse_q_rope ? (size_t)(d.n_b + kChunk) * d.half * sizeof(float2) : 0;
+}
+
+static size_t route_ws_bytes(const Derived& d) {
+  size_t n = d.route_max ? route_max_ws_bytes(d)                               // + group-candidate scores, prefilter tables
+                         : (size_t)d.B * d.Hkv * d.n_b * d.n_b * sizeof(float);  // chunk-score matrix
+  return (n + 255) & ~(size_t)255;
+}
+
 static size_t score_ws_bytes(const Derived& d) {
-  if (d.route_max) return route_max_ws_bytes(d);  // + group-candidate scores and the tensor-core prefilter's tables
-  return (size_t)d.B * d.Hkv * d.n_b * d.n_b * sizeof(float);  // chunk-score matrix
+  return route_ws_bytes(d) + rope_tables_bytes(d);
 }
 
 }  // namespace hga
@@ -247,7 +258,14 @@ static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* 
   d.tw0 = t_begin; d.tw1 = t_end;
   d.jb = (int)(t_begin / kChunk);
   d.nj = (int)((t_end + kChunk - 1) / kChunk) - d.jb;
-  if (!b->q_raw || !b->k_raw || !b->v || !b->q_rot || !b->k_rot || !b->q_pooled || !b->chunk_sum || !b->out ||
+  const bool fuse = d.fuse_q_rope != 0;
+  if (fuse) {
+    // N2: whole blocks, the pooled-query rule, the persistent tcgen05 kernel (see hga_flag in hga.h)
+    if (!d.bf16_io || d.route_max || t_begin % kChunk != 0 || t_end % kChunk != 0 ||
+        (p->attend_impl != HGA_ATTEND_AUTO && p->attend_impl != HGA_ATTEND_TCGEN05))
+      return HGA_ERR_UNSUPPORTED;
+  }
+  if (!b->q_raw || !b->k_raw || !b->v || (!fuse && !b->q_rot) || !b->k_rot || !b->q_pooled || !b->chunk_sum || !b->out ||
       !b->chunk_idx)
     return HGA_ERR_INVALID_ARG;
   if (d.Kg > 0 && (!b->group_sum || !b->group_idx)) return HGA_ERR_INVALID_ARG;
@@ -259,7 +277,14 @@ static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* 
   cudaStream_t cs = (cudaStream_t)stream;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[0], cs));
   // S0 + S1 in one launch: the K tiles and Q tiles of a (batch, chunk) row share the position tables
-  st = launch_rope_summaries(d, f, b->q_raw, b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum, b->group_sum, cs);
+  float2* rope_a = reinterpret_cast<float2*>((unsigned char*)b->workspace + route_ws_bytes(d));
+  float2* rope_b = rope_a + (size_t)d.n_b * d.half;
+  if (fuse) {
+    st = launch_rope_tables(d, f, rope_a, rope_b, cs);
+    if (st != HGA_OK) return st;
+  }
+  st = launch_rope_summaries(d, f, b->q_raw, fuse ? nullptr : b->q_rot, b->q_pooled, b->k_raw, b->k_rot, b->chunk_sum,
+                             b->group_sum, cs);
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[1], cs));
   if (d.route_max) {
@@ -273,7 +298,8 @@ static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* 
   }
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[2], cs));
-  st = attend_dispatch(d, p->attend_impl, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, cs);
+  if (fuse) st = launch_attend_tc2_rawq(d, b->q_raw, b->k_rot, b->v, b->group_idx, b->out, b->lse, rope_a, rope_b, cs);
+  else st = attend_dispatch(d, p->attend_impl, b->q_rot, b->k_rot, b->v, b->group_idx, b->out, b->lse, cs);
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[3], cs));
   return HGA_OK;

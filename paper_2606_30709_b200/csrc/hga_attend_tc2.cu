@@ -73,6 +73,11 @@ struct Tc2Params {
   int n_items;
   float scale_log2;   // softmax_scale * log2(e)
   int out_bf16;
+  // kRawQ (N2, the Q_rot round trip removed): tmQ maps the UN-rotated queries and the epilogue warpgroup rotates every Q
+  // tile in shared memory before its first Q K^T.  (cos, sin) of position pos0 + 64 j + t for pair i is the product of
+  // rope_a[j][i] (the block's first position) and rope_b[t][i] (offset t inside the block), both from launch_rope_tables.
+  const float2* rope_a;  // [n_b][D/2]
+  const float2* rope_b;  // [64][D/2]
 };
 
 template <int D>
@@ -89,7 +94,7 @@ struct Smem2 {
   // barrier ids
   static constexpr int QFULL = 0, QEMPTY = 2, SFULL = 4, PFULL = 6, OFULL = 8, OEMPTY = 10, LFULL = 12, LEMPTY = 14,
                        LISTFULL = 16, LISTEMPTY = 18, KFULL = 20, KEMPTY = KFULL + kStages, VFULL = KEMPTY + kStages,
-                       VEMPTY = VFULL + kStages, PFULLB = VEMPTY + kStages, kNumBars = PFULLB + 2;
+                       VEMPTY = VFULL + kStages, PFULLB = VEMPTY + kStages, QROT = PFULLB + 2, kNumBars = QROT + 2;
   static constexpr int kMisc = kBar + 8 * kNumBars;  // tmem base (4 B), n_pieces[2]
   static constexpr int kInvL = kMisc + 16;           // 2 tiles x 128 rows fp32: 1/l (split mode: l), then m (split mode)
   static constexpr int kList = kInvL + 4 * 128 * 4;  // 2 x list_cap ints
@@ -117,7 +122,7 @@ __device__ __forceinline__ Item decode_item(int it, const Tc2Params& prm) {
 }
 
 // kSplit: one query tile per item (G <= 2), see the MMA issuer.  kPad: some tile holds a padding head (odd G).
-template <int D, bool kSplit, bool kPad>
+template <int D, bool kSplit, bool kPad, bool kRawQ>
 __global__ void __launch_bounds__(kThreads, 1)
 attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
@@ -139,6 +144,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     for (int t = 0; t < 2; ++t) {
       mbar_init(BAR(L::QFULL + t), 1);
       mbar_init(BAR(L::QEMPTY + t), 1);
+      mbar_init(BAR(L::QROT + t), 4);  // the four epilogue warps, after rotating the tile (kRawQ)
       mbar_init(BAR(L::SFULL + t), 1);
       mbar_init(BAR(L::PFULL + t), 4);
       mbar_init(BAR(L::PFULLB + t), 4);
@@ -257,8 +263,70 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int colw = prm.out_bf16 ? 64 : 32;  // columns per 128-byte staging row
     uint32_t o_cnt[2] = {0, 0};  // items drained per tile
     const uint64_t pol_o = policy_evict_first();
+    // kRawQ: RoPE on the Q tiles of an item, in place in shared memory, as soon as the raw tile has landed (during the
+    // previous item's last key-tile step, when this warpgroup is idle) and before the issuer's first Q K^T of the tile.
+    // A thread takes (token, 8 pairs) of both heads of the tile: x = columns [8 pc, 8 pc + 8), y = the same + D/2; the
+    // arithmetic is rope_stream_kernel's (fp32 FMA, one RNE rounding to bf16).
+    uint32_t qr_cnt[2] = {0, 0};  // Q tiles rotated per slot
+    auto rotate_item = [&](const Item& im) {
+      constexpr int PCS = D / 16;  // 8-pair pieces per row
+      const int eid = e * 32 + lane;
+      for (int t = 0; t < (kSplit ? 2 : im.nt); ++t) {
+        mbar_wait(BAR(L::QFULL + t), qr_cnt[t] & 1u);
+        ++qr_cnt[t];
+        unsigned char* qt = smem + L::kQ + t * L::kTileBytes;
+        const float2* ta = prm.rope_a + (size_t)im.j * (D / 2);
+        for (int task = eid; task < 64 * PCS; task += 128) {
+          const int tok = task / PCS, pc = task % PCS;
+          float2 cs[8];
+#pragma unroll
+          for (int h4 = 0; h4 < 2; ++h4) {
+            const float4* pa = reinterpret_cast<const float4*>(ta + pc * 8 + h4 * 4);
+            const float4* pb = reinterpret_cast<const float4*>(prm.rope_b + (size_t)tok * (D / 2) + pc * 8 + h4 * 4);
+            const float4 a01 = __ldg(pa), a23 = __ldg(pa + 1), b01 = __ldg(pb), b23 = __ldg(pb + 1);
+            const float2 a[4] = {make_float2(a01.x, a01.y), make_float2(a01.z, a01.w), make_float2(a23.x, a23.y),
+                                 make_float2(a23.z, a23.w)};
+            const float2 b[4] = {make_float2(b01.x, b01.y), make_float2(b01.z, b01.w), make_float2(b23.x, b23.y),
+                                 make_float2(b23.z, b23.w)};
+#pragma unroll
+            for (int u = 0; u < 4; ++u)  // (cos, sin)(alpha + beta)
+              cs[4 * h4 + u] = make_float2(fmaf(a[u].x, b[u].x, -(a[u].y * b[u].y)), fmaf(a[u].y, b[u].x, a[u].x * b[u].y));
+          }
+          // x chunk: column block 0, chunk pc;  y chunk: D = 128 -> column block 1, chunk pc;  D = 64 -> chunk pc + 4
+          const int ycb = (D == 128) ? 1 : 0, ych = (D == 128) ? pc : pc + 4;
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            const int rr = hh * 64 + tok;
+            uint4* px = reinterpret_cast<uint4*>(qt + rr * 128 + ((pc ^ (rr & 7)) << 4));
+            uint4* py = reinterpret_cast<uint4*>(qt + ycb * L::kHalfBytes + rr * 128 + ((ych ^ (rr & 7)) << 4));
+            const uint4 xv = *px, yv = *py;
+            const uint32_t xw[4] = {xv.x, xv.y, xv.z, xv.w}, yw[4] = {yv.x, yv.y, yv.z, yv.w};
+            uint32_t xo[4], yo[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const float x0 = __uint_as_float(xw[u] << 16), x1 = __uint_as_float(xw[u] & 0xFFFF0000u);
+              const float y0 = __uint_as_float(yw[u] << 16), y1 = __uint_as_float(yw[u] & 0xFFFF0000u);
+              const float2 c0 = cs[2 * u], c1 = cs[2 * u + 1];
+              xo[u] = cvt_bf16x2(fmaf(x0, c0.x, -(y0 * c0.y)), fmaf(x1, c1.x, -(y1 * c1.y)));
+              yo[u] = cvt_bf16x2(fmaf(y0, c0.x, x0 * c0.y), fmaf(y1, c1.x, x1 * c1.y));
+            }
+            *px = make_uint4(xo[0], xo[1], xo[2], xo[3]);
+            *py = make_uint4(yo[0], yo[1], yo[2], yo[3]);
+          }
+        }
+        fence_proxy_async();  // the rotated tile becomes visible to the tensor core's shared-memory reads
+        __syncwarp();
+        if (lane == 0) mbar_arrive(BAR(L::QROT + t));
+      }
+    };
+    if constexpr (kRawQ) {
+      if ((int)blockIdx.x < prm.n_items) rotate_item(decode_item(blockIdx.x, prm));
+    }
     for (int it = blockIdx.x; it < prm.n_items; it += gridDim.x) {
       const Item im = decode_item(it, prm);
+      if constexpr (kRawQ) {
+        if (it + (int)gridDim.x < prm.n_items) rotate_item(decode_item(it + gridDim.x, prm));
+      }
       for (int t = 0; t < im.nt; ++t) {
         mbar_wait(BAR(L::OFULL + t), o_cnt[t] & 1u);
         mbar_wait(BAR(L::LFULL + t), o_cnt[t] & 1u);
@@ -511,7 +579,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         // first Q K^T of virtual tile t for an item of np pieces whose key tile 0 is global tile b0
         auto first_qk = [&](int t, int np, uint32_t b0) {
           const int nt_ = (np + kPPT - 1) / kPPT;
-          mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+          mbar_wait(BAR((kRawQ ? L::QROT : L::QFULL) + t), q_cnt[t] & 1u);
           ++q_cnt[t];
           if (t < nt_) {
             const int ks = (int)((b0 + (uint32_t)t) % L::kStages);
@@ -646,7 +714,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         auto first_qk = [&](auto T) {
           constexpr int t = decltype(T)::value;
           if (t < nt) {
-            mbar_wait(BAR(L::QFULL + t), 0);
+            mbar_wait(BAR((kRawQ ? L::QROT : L::QFULL) + t), 0);
             ++q_cnt[t];
             tc_fence_after();
             qk(T, std::integral_constant<int, 0>{}, min(kPPT, n_pieces) * 16);
@@ -713,7 +781,7 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
               }
               if (more && t < nt_qk) {
                 if (last) {
-                  mbar_wait(BAR(L::QFULL + t), q_cnt[t] & 1u);
+                  mbar_wait(BAR((kRawQ ? L::QROT : L::QFULL) + t), q_cnt[t] & 1u);
                   ++q_cnt[t];
                   tc_fence_after();
                 }
@@ -754,9 +822,10 @@ attend_tc2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   }
 }
 
+// rope_a / rope_b non-null: q holds the UN-rotated queries and the kernel applies RoPE itself (kRawQ)
 template <int D>
 hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const void* v, const int32_t* gi, void* out,
-                        float* lse, cudaStream_t s) {
+                        float* lse, const float2* rope_a, const float2* rope_b, cudaStream_t s) {
   using L = Smem2<D>;
   Tc2Params prm;
   prm.B = d.B; prm.Hq = d.Hq; prm.Hkv = d.Hkv; prm.N = d.N; prm.n_b = d.n_b; prm.G = d.G;
@@ -768,6 +837,8 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
   prm.list_cap = max_key_pieces(d.F, d.L_eff, d.gs, d.Kg);
   prm.scale_log2 = d.scale * 1.4426950408889634f;
   prm.out_bf16 = d.bf16_out ? 1 : 0;
+  prm.rope_a = rope_a;
+  prm.rope_b = rope_b;
   const long long n_items = (long long)d.B * d.Hkv * d.nj * prm.ctas_per_unit;
   const size_t smem = (size_t)L::kList + 2 * sizeof(int) * (size_t)prm.list_cap;
   if (smem > 227 * 1024 || n_items >= (1ll << 31)) return HGA_ERR_UNSUPPORTED;
@@ -783,8 +854,10 @@ hga_status launch_tc2_t(const Derived& d, const void* q, const void* k, const vo
   if (!ok) return HGA_ERR_CUDA;
   const int n_sm = current_sm_count();
   if (n_sm <= 0) return HGA_ERR_CUDA;
-  auto kern = prm.split ? attend_tc2_kernel<D, true, true>
-                        : (d.G % 2 ? attend_tc2_kernel<D, false, true> : attend_tc2_kernel<D, false, false>);
+  const bool raw = rope_a != nullptr && rope_b != nullptr;
+  auto kern = prm.split ? (raw ? attend_tc2_kernel<D, true, true, true> : attend_tc2_kernel<D, true, true, false>)
+              : d.G % 2 ? (raw ? attend_tc2_kernel<D, false, true, true> : attend_tc2_kernel<D, false, true, false>)
+                        : (raw ? attend_tc2_kernel<D, false, false, true> : attend_tc2_kernel<D, false, false, false>);
   HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int grid = (int)(n_items < n_sm ? n_items : n_sm);
   kern<<<grid, kThreads, smem, s>>>(tmQ, tmK, tmV, tmO, gi, lse, prm);
@@ -804,8 +877,17 @@ extern "C" __attribute__((visibility("default"))) int hga_debug_trace(long long*
 hga_status launch_attend_tc2(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                              void* out, float* lse, cudaStream_t s) {
   if (!d.bf16_io) return HGA_ERR_UNSUPPORTED;
-  return d.D == 128 ? launch_tc2_t<128>(d, q, k, v, group_idx, out, lse, s)
-                    : launch_tc2_t<64>(d, q, k, v, group_idx, out, lse, s);
+  return d.D == 128 ? launch_tc2_t<128>(d, q, k, v, group_idx, out, lse, nullptr, nullptr, s)
+                    : launch_tc2_t<64>(d, q, k, v, group_idx, out, lse, nullptr, nullptr, s);
+}
+
+// N2: the same kernel on UN-rotated queries; RoPE is applied to every Q tile inside the kernel from the two position
+// tables of launch_rope_tables (rope_a: [n_b][D/2], rope_b: [64][D/2]), so Q_rot never goes through HBM.
+hga_status launch_attend_tc2_rawq(const Derived& d, const void* q_raw, const void* k, const void* v, const int32_t* group_idx,
+                                  void* out, float* lse, const float2* rope_a, const float2* rope_b, cudaStream_t s) {
+  if (!d.bf16_io || !rope_a || !rope_b) return HGA_ERR_UNSUPPORTED;
+  return d.D == 128 ? launch_tc2_t<128>(d, q_raw, k, v, group_idx, out, lse, rope_a, rope_b, s)
+                    : launch_tc2_t<64>(d, q_raw, k, v, group_idx, out, lse, rope_a, rope_b, s);
 }
 
 }  // namespace hga

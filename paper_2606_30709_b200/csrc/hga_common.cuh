@@ -29,6 +29,7 @@ struct Derived {
   long long pos0;
   long long pos_mod;  // RoPE position wrap; 0 = off
   float scale;              // softmax scale
+  int fuse_q_rope;          // N2: hga_prefill does not materialise q_rot; S4 rotates its query tiles (HGA_FLAG_FUSE_Q_ROPE)
   int route_max;            // N3: block score = max over per-query scores (R19) instead of the pooled-query score
                             // (the hga_route_mode value: 1 = tensor-core prefilter where eligible, 2 = fp64 pipe only)
   bool bf16_io, bf16_out;
@@ -108,6 +109,9 @@ hga_status launch_attend_simt(const Derived& d, const void* q, const void* k, co
                               void* out, float* lse, cudaStream_t s);
 hga_status launch_attend_tc2(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                              void* out, float* lse, cudaStream_t s);
+hga_status launch_attend_tc2_rawq(const Derived& d, const void* q_raw, const void* k, const void* v, const int32_t* group_idx,
+                                  void* out, float* lse, const float2* rope_a, const float2* rope_b, cudaStream_t s);
+hga_status launch_rope_tables(const Derived& d, const RopeFreq& f, float2* rope_a, float2* rope_b, cudaStream_t s);
 hga_status launch_attend_pair(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,
                               void* out, float* lse, cudaStream_t s);
 hga_status launch_attend_tc(const Derived& d, const void* q, const void* k, const void* v, const int32_t* group_idx,

@@ -52,7 +52,7 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
 
 struct RsParams {
   const void* q_raw;
-  void* q_rot;
+  void* q_rot;    // nullable: skip the store
   float* pooled;  // nullable
   const void* k_raw;
   void* k_rot;       // nullable: skip the store
@@ -213,7 +213,7 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
       T* dst = nullptr;
       if (is_k) {
         if (p.k_rot) dst = (T*)p.k_rot + (((size_t)b * p.HK + r) * p.N + (size_t)j * kChunk + tok) * D;
-      } else {
+      } else if (p.q_rot) {  // nullptr: the rotated queries are only pooled (N2: S4 rotates its Q tiles itself)
         dst = (T*)p.q_rot + (((size_t)b * p.HQ + (r - p.HK)) * p.N + (size_t)j * kChunk + tok) * D;
       }
       if (dst && in_window) {
@@ -335,6 +335,24 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
   }
 }
 
+// N2 position tables for the in-kernel RoPE of S4: rope_a[j][i] = (cos, sin) of the first position of block j (wrapped like
+// rope_stream_kernel wraps it), rope_b[t][i] = (cos, sin) of offset t, both with cos_sin_f32's accuracy; the angle of
+// token 64 j + t is their sum, so S4 needs 512 bytes per block plus one 64-row table that stays in L1.
+__global__ void rope_tables_kernel(const __grid_constant__ RopeFreq f, float2* __restrict__ rope_a, float2* __restrict__ rope_b,
+                                   int n_b, int half, long long pos0, long long pos_mod) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n_a = n_b * half;
+  if (idx < n_a) {
+    const int j = idx / half, i = idx % half;
+    long long pos_first = pos0 + (long long)j * kChunk;
+    if (pos_mod > 0) pos_first %= pos_mod;
+    rope_a[idx] = cos_sin_f32((double)pos_first, f.turns[i]);
+  } else if (idx < n_a + kChunk * half) {
+    const int t = (idx - n_a) / half, i = (idx - n_a) % half;
+    rope_b[idx - n_a] = cos_sin_f32((double)t, f.turns[i]);
+  }
+}
+
 template <typename T, int D>
 hga_status launch_stream_t(const RopeFreq& f, RsParams p, long long rows, cudaStream_t s) {
   using C = RsCfg<T, D>;
@@ -383,6 +401,12 @@ hga_status launch_rope_summaries(const Derived& d, const RopeFreq& f, const void
   p.k_raw = k_raw; p.k_rot = k_rot; p.chunk_sum = chunk_sum; p.group_sum = group_sum;
   p.HK = d.Hkv;
   return launch_stream(d, f, p, s);
+}
+
+hga_status launch_rope_tables(const Derived& d, const RopeFreq& f, float2* rope_a, float2* rope_b, cudaStream_t s) {
+  const int half = d.D / 2, total = (d.n_b + kChunk) * half;
+  rope_tables_kernel<<<(total + 255) / 256, 256, 0, s>>>(f, rope_a, rope_b, d.n_b, half, d.pos0, d.pos_mod);
+  return launch_status();
 }
 
 hga_status launch_rope(const Derived& d, const RopeFreq& f, const void* x_raw, int n_heads, void* x_rot, float* pooled,

@@ -66,6 +66,7 @@ def main():
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--impl", type=int, default=0, help="hga_attend_impl (0 auto, 2 persistent, 4 CTA pair)")
     ap.add_argument("--trace", action="store_true", help="print the HGA_S4_TRACE timeline (needs a trace build)")
+    ap.add_argument("--out-bf16", action="store_true", help="bf16 output rows instead of fp32")
     ap.add_argument("--route-max", action="store_true", help="time hga_route_max under HGA_ROUTE_MAX and HGA_ROUTE_MAX_FP64")
     args = ap.parse_args()
     import numpy as np
@@ -82,7 +83,7 @@ def main():
     dq, dk, dv = (torch.from_numpy(a).to(dt).cuda() for a in (q, k, v))
     if args.route_max:
         return route_max_probe(B, w, dq, dk, dv, args.reps)
-    p = B.params_from_workload(w, attend_impl=args.impl)
+    p = B.params_from_workload(w, attend_impl=args.impl, out_dtype=B.HGA_BF16 if args.out_bf16 else B.HGA_F32)
     buf = B.PrefillBuffers.allocate(p)
     for _ in range(3):
         B.hga_prefill(p, dq, dk, dv, buf)

@@ -113,8 +113,9 @@ def check_against_oracle(w: W.Workload, q, k, v, p, buf, slices, blocks, check_i
             for j in blocks[:: max(1, len(blocks) // 8)]:
                 qo = oracle.round_io(oracle.rope(q[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C], op.pos0 + j * C, op.base,
                                                  op.pos_mod), op.io_bf16)
-                qg = buf.q_rot[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C].float().cpu().numpy().astype(np.float64)
-                worst["q_rot"] = max(worst["q_rot"], float(np.abs(qg - qo).max()))
+                if buf.q_rot is not None:  # not materialised under FLAG_FUSE_Q_ROPE
+                    qg = buf.q_rot[b, kh * G:(kh + 1) * G, j * C:(j + 1) * C].float().cpu().numpy().astype(np.float64)
+                    worst["q_rot"] = max(worst["q_rot"], float(np.abs(qg - qo).max()))
         g_out = buf.out[b, kh * G:(kh + 1) * G].float().cpu().numpy().astype(np.float64)  # [G,N,D]
         g_lse = buf.lse[b, kh * G:(kh + 1) * G].cpu().numpy().astype(np.float64)
         kv64 = v[b, kh].astype(np.float64)

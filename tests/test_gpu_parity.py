@@ -481,6 +481,61 @@ def test_route_max_tensor_core_prefilter_many_tied_queries():
     parity.assert_report(rep, w, len(blocks))
 
 
+# ---------------------------------------------------------------------------------------------------------------
+# N2: HGA_FLAG_FUSE_Q_ROPE -- q_rot is never written; S0 only pools, S4 reads q_raw and rotates its query tiles in
+# shared memory.  Against the oracle on every block, and against the unfused path (same lists bit for bit; outputs equal
+# up to the rare one-step bf16 difference of a rotated query, far inside the output tolerance).
+# ---------------------------------------------------------------------------------------------------------------
+FUSED = [
+    # name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L, pos0, pos_mod
+    ("fz_d128_g8", 1, 2048, 16, 2, 128, 1e6, 6, 24, 1, 1, 0, 0),
+    ("fz_d128_g3_f2l3", 2, 1536, 6, 2, 128, 1e6, 5, 7, 2, 3, 0, 0),       # odd G: a padding head in the last tile
+    ("fz_d64_g2", 1, 2048, 4, 2, 64, 1e4, 5, 11, 1, 1, 0, 0),             # split mode: one query tile on both warpgroups
+    ("fz_d64_g1", 2, 1024, 4, 4, 64, 1e4, 4, 8, 1, 1, 0, 0),              # split + padding
+    ("fz_d64_g6", 1, 2048, 6, 1, 64, 1e4, 6, 12, 1, 2, 0, 0),
+    ("fz_d128_g4_pos0", 1, 2048, 8, 2, 128, 1e6, 6, 24, 1, 1, 40000 * 64, 0),
+    ("fz_d128_g2_wrap", 1, 4096, 4, 2, 128, 1e4, 6, 24, 1, 1, 0, 2048),   # positions wrap in mid-sequence
+    ("fz_smalllm_12k", 1, 12288, 6, 2, 64, 1e4, 16, 32, 1, 1, 0, 0),      # >= 4 items per persistent CTA
+]
+
+
+@pytest.mark.parametrize("cfg", FUSED, ids=[c[0] for c in FUSED])
+def test_fused_q_rope_full_parity(cfg):
+    name, B, N, Hq, Hkv, D, base, Kc, Kg, F, L, pos0, pos_mod = cfg
+    w = W.Workload(name, B, N, Hq, Hkv, D, "bf16", base, n_sink=F, n_local=L, topk_chunks=Kc, topk_groups=Kg, n_clusters=8,
+                   pos0=pos0, rope_pos_mod=pos_mod)
+    q, k, v = W.generate(w, 41)
+    p, buf = parity.run_gpu(w, q, k, v, flags=hga.binding.FLAG_FUSE_Q_ROPE)
+    assert buf.q_rot is None
+    blocks = np.arange(w.n_blocks) if N <= 4096 else _sample_blocks(w.n_blocks, 24, 4)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, _all_slices(w), blocks)
+    parity.assert_report(rep, w, len(blocks) * B * Hkv)
+    p0, buf0 = parity.run_gpu(w, q, k, v)
+    for a, b in zip(_route_outputs(buf), _route_outputs(buf0)):
+        assert torch.equal(a, b)
+    assert torch.equal(buf.k_rot, buf0.k_rot) and torch.equal(buf.q_pooled, buf0.q_pooled)
+    diff = (buf.out - buf0.out).abs()
+    assert float(diff.max()) <= 5e-3, float(diff.max())
+    assert float((diff > 0).float().mean()) < 0.2      # most rows see exactly the same rotated queries
+
+
+def test_fused_q_rope_c5_whole_slice_and_rejections():
+    """BASELINE.json configs[4] at full size through the fused path: one whole (batch, kv head) slice against the oracle;
+    then the argument checks of the flag."""
+    w = W.get("c5")
+    q, k, v = W.generate(w, 0)
+    p, buf = parity.run_gpu(w, q, k, v, flags=hga.binding.FLAG_FUSE_Q_ROPE)
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [(0, 2)], np.arange(w.n_blocks))
+    parity.assert_report(rep, w, w.n_blocks)
+    assert torch.isfinite(buf.out).all()
+    dq, dk, dv = parity.to_device(w, (q, k, v))
+    for bad in (dict(route_mode=hga.binding.ROUTE_MAX), dict(attend_impl=ATTEND_SIMT), dict(attend_impl=ATTEND_TCGEN05_ITEM)):
+        with pytest.raises(RuntimeError, match="UNSUPPORTED"):
+            hga.hga_prefill(p.replace(**bad), dq, dk, dv)
+    with pytest.raises(RuntimeError, match="INVALID_ARG"):
+        hga.hga_prefill(p.replace(flags=2), dq, dk, dv)
+
+
 def test_route_max_mode_c5_full_size_sampled():
     """The max rule at BASELINE.json configs[4] (64K, Qwen3 head shape): sampled blocks of two slices against the oracle."""
     w = dataclasses.replace(W.get("c5"), route_max=True)
