@@ -501,6 +501,19 @@ def run_ours(args, w):
                                 "return the same lists bit for bit; the default pooled-query rule is stages.S2S3_route"}
             hga.hga_prefill(p, dq, dk, dv, buf)  # restore the default rule's lists in buf
             torch.cuda.synchronize()
+            # N2: hga_prefill with HGA_FLAG_FUSE_Q_ROPE (q_rot never written; S4 rotates its query tiles itself)
+            pf = p.replace(flags=hga.binding.FLAG_FUSE_Q_ROPE)
+            buf_f = hga.binding.PrefillBuffers.allocate(pf)
+            for _ in range(3):
+                hga.hga_prefill(pf, dq, dk, dv, buf_f)
+            torch.cuda.synchronize()
+            fm = np.median(np.array([hga.hga_prefill_profile(pf, dq, dk, dv, buf_f) for _ in range(10)]), axis=0)
+            variants["fused_q_rope_stage_ms"] = {"S0S1": float(fm[0]), "S2S3": float(fm[1]), "S4": float(fm[2]),
+                                                 "sum": float(fm.sum())}
+            variants["fused_q_rope_what"] = ("hga_prefill with HGA_FLAG_FUSE_Q_ROPE (N2): S0 pools the rotated queries without "
+                                             "storing them, S4 reads q_raw and applies RoPE to its query tiles in shared memory; "
+                                             "compare with stages.* of the default path -- built, parity-green and slower")
+            del buf_f
         except Exception as e:  # a variant must never sink the headline line
             variants = {"error": str(e)}
 
