@@ -50,6 +50,32 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
                : "memory");
 }
 
+// 8 consecutive elements of a staged tile as fp32, through a 32-bit shared-space address (a generic pointer into the
+// dynamic shared array makes ptxas re-derive the shared window base -- S2R SR_CgaCtaId + LEA -- at every tile)
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+  return r;
+}
+template <typename T>
+__device__ __forceinline__ void load8_shared(uint32_t addr, float (&v)[8]);
+template <>
+__device__ __forceinline__ void load8_shared<float>(uint32_t addr, float (&v)[8]) {
+  const uint4 a = lds128(addr), b = lds128(addr + 16);
+  v[0] = __uint_as_float(a.x); v[1] = __uint_as_float(a.y); v[2] = __uint_as_float(a.z); v[3] = __uint_as_float(a.w);
+  v[4] = __uint_as_float(b.x); v[5] = __uint_as_float(b.y); v[6] = __uint_as_float(b.z); v[7] = __uint_as_float(b.w);
+}
+template <>
+__device__ __forceinline__ void load8_shared<__nv_bfloat16>(uint32_t addr, float (&v)[8]) {
+  const uint4 r = lds128(addr);
+  const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    v[2 * i] = __uint_as_float(w[i] << 16);  // bf16 -> fp32 is exact
+    v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+  }
+}
+
 struct RsParams {
   const void* q_raw;
   void* q_rot;    // nullable: skip the store
@@ -67,6 +93,9 @@ struct RsParams {
   int tpr;     // tiles per row = HK + HQ
   long long pos0, pos_mod;
   long long total_tiles;  // rows * tpr
+  // host-derived copies of per-tile tests (uniform; the 64-bit null tests and the power-of-two test were a measurable
+  // share of the consumers' instruction stream): stores wanted, pooling wanted, PG - 1 when PG is a power of two else -1
+  int store_q, store_k, pool_q, pg_mask;
 };
 
 // First tile of CTA `c` when `total` tiles are split over `n` CTAs at unit boundaries (a K tile, or PG Q tiles).
@@ -110,7 +139,10 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
   using C = RsCfg<T, D>;
   constexpr int half = C::kHalf, OCT = C::kOct, S = C::kStages, NW = C::kCWarps;
   extern __shared__ __align__(128) unsigned char smem[];
-  const uint32_t sbase = smem_u32(smem);
+  uint32_t sbase = smem_u32(smem);
+  // opaque to ptxas, which otherwise re-derives the shared-window base from SR_CgaCtaId (an S2R) at every barrier of every
+  // tile (4 % of the kernel's stall samples on those S2R / LEA pairs)
+  asm volatile("mov.u32 %0, %0;" : "+r"(sbase));
   float* part_base = reinterpret_cast<float*>(smem + C::kPart);
   double2* mid_base = reinterpret_cast<double2*>(smem + C::kMid);
   double* s_turns = reinterpret_cast<double*>(smem + C::kTurns);
@@ -195,10 +227,10 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
     }
     const int s = k % S;
     mbar_wait(FULL(s), (uint32_t)(k / S) & 1u);
-    const T* rowp = reinterpret_cast<const T*>(smem + C::kTiles + s * C::kTileBytes) + tok * D;
+    const uint32_t rowa = sbase + (uint32_t)(C::kTiles + s * C::kTileBytes + (tok * D + i0) * (int)sizeof(T));
     float a[8], bb[8], ra[8], rb[8];
-    Io<T>::load8(rowp + i0, a);
-    Io<T>::load8(rowp + half + i0, bb);
+    load8_shared<T>(rowa, a);
+    load8_shared<T>(rowa + half * (uint32_t)sizeof(T), bb);
     __syncwarp();
     if (lane == 0) mbar_arrive(EMPTY(s));  // the values are in registers: the stage can be refilled
 #pragma unroll
@@ -209,19 +241,16 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
     }
     const int t_abs = j * kChunk + tok;
     const bool in_window = t_abs >= p.tw0 && t_abs < p.tw1;
-    {
-      T* dst = nullptr;
-      if (is_k) {
-        if (p.k_rot) dst = (T*)p.k_rot + (((size_t)b * p.HK + r) * p.N + (size_t)j * kChunk + tok) * D;
-      } else if (p.q_rot) {  // nullptr: the rotated queries are only pooled (N2: S4 rotates its Q tiles itself)
-        dst = (T*)p.q_rot + (((size_t)b * p.HQ + (r - p.HK)) * p.N + (size_t)j * kChunk + tok) * D;
-      }
-      if (dst && in_window) {
-        Io<T>::store8(dst + i0, ra);
-        Io<T>::store8(dst + half + i0, rb);
-      }
+    // store_q == 0: the rotated queries are only pooled (N2: S4 rotates its Q tiles itself)
+    if ((is_k ? p.store_k : p.store_q) && in_window) {
+      // token rows fit 32 bits (launch_stream checks B * heads * N < 2^31): one widening multiply per address
+      T* base = is_k ? (T*)p.k_rot : (T*)p.q_rot;
+      const int head = is_k ? b * p.HK + r : b * p.HQ + (r - p.HK);
+      T* dst = base + (size_t)(unsigned)(head * p.N + t_abs) * D;
+      Io<T>::store8(dst + i0, ra);
+      Io<T>::store8(dst + half + i0, rb);
     }
-    const bool pool = !is_k && p.pooled != nullptr;
+    const bool pool = !is_k && p.pool_q;
     if (pool && in_window) {
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
@@ -229,7 +258,10 @@ rope_stream_kernel(const __grid_constant__ RopeFreq f, const __grid_constant__ R
         acc[8 + u] += rb[u];
       }
     }
-    const bool unit_end = pool && ((r - p.HK + 1) % p.PG == 0);
+    // the runtime modulo is 25 instructions and was 12 % of the kernel's stall samples (ncu source page); G is a power of
+    // two in every model shape of the paper
+    const int q_done = r - p.HK + 1;
+    const bool unit_end = pool && (p.pg_mask >= 0 ? (q_done & p.pg_mask) == 0 : q_done % p.PG == 0);
     float* part = part_base + (size_t)pb * NW * 2 * D;
     if (is_k) {
       // sums over the kTpw tokens of this warp (all inside one 16-token group), fixed order
@@ -360,6 +392,10 @@ hga_status launch_stream_t(const RopeFreq& f, RsParams p, long long rows, cudaSt
   if (n_sm <= 0) return HGA_ERR_CUDA;
   p.tpr = p.HK + p.HQ;
   p.total_tiles = rows * p.tpr;
+  p.store_q = p.q_rot != nullptr;
+  p.store_k = p.k_rot != nullptr;
+  p.pool_q = p.pooled != nullptr;
+  p.pg_mask = (p.PG & (p.PG - 1)) == 0 ? p.PG - 1 : -1;
   const long long units = rows * (p.HK + (p.HQ ? p.HQ / p.PG : 0));
   const int ctas_per_sm = C::kCtasPerSm;
   const long long cap = (long long)n_sm * ctas_per_sm;
@@ -373,6 +409,7 @@ hga_status launch_stream_t(const RopeFreq& f, RsParams p, long long rows, cudaSt
 
 hga_status launch_stream(const Derived& d, const RopeFreq& f, const RsParams& p, cudaStream_t s) {
   const long long rows = (long long)d.B * d.nj;
+  if ((long long)d.B * (p.HQ > p.HK ? p.HQ : p.HK) * d.N >= (1ll << 31)) return HGA_ERR_UNSUPPORTED;  // 32-bit token rows
   if (d.bf16_io) {
     return d.D == 128 ? launch_stream_t<__nv_bfloat16, 128>(f, p, rows, s) : launch_stream_t<__nv_bfloat16, 64>(f, p, rows, s);
   }
