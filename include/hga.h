@@ -193,6 +193,22 @@ HGA_API hga_status hga_route(const hga_params* p, const float* q_pooled, const f
                              size_t workspace_bytes, void* stream);
 
 /*
+ * hga_route without a workspace argument and without any allocation, for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it): the chunk-score matrix lives in a static device
+ * array of HGA_ROUTE_STATIC_MAX_BYTES inside the library (every GPU that loads the library holds it until the process
+ * exits).  Same arguments, outputs and results as hga_route, bit for bit.  Limit: batch * n_kv_heads * (seq/chunk)^2 * 4
+ * bytes <= HGA_ROUTE_STATIC_MAX_BYTES (BASELINE.json configs[4], 64K tokens x 4 KV heads, fits exactly); a larger problem
+ * returns HGA_ERR_WORKSPACE and launches nothing -- use hga_route with a caller-owned workspace.  HGA_ROUTE_MEAN only.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress, which may load the module: make one
+ * call before starting a graph capture).  All calls share the array: calls that overlap on the GPU (different streams,
+ * concurrently replayed graphs) race; calls ordered on one stream do not.  Nothing in it has to be cleared between calls.
+ */
+#define HGA_ROUTE_STATIC_MAX_BYTES (16u << 20)
+HGA_API hga_status hga_route_static(const hga_params* p, const float* q_pooled, const float* chunk_sum,
+                                    const float* group_sum, int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks,
+                                    int32_t* group_idx, float* group_score, int32_t* n_groups, void* stream);
+
+/*
  * S2 + S3 under HGA_ROUTE_MAX / HGA_ROUTE_MAX_FP64 (p->route_mode must be one of them): the same candidate sets, budgets, tie rule and
  * outputs as hga_route, with score(candidate) = max over the 64*G rotated queries of block j (all heads of the GQA
  * group, read from q_rot [B,H_q,N,D] in io_dtype) of <q, summary> in fp64.  hga_route itself rejects HGA_ROUTE_MAX

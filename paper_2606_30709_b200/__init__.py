@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     hga_prefill_window,
     hga_rope,
     hga_route,
+    hga_route_static,
     hga_validate,
     hga_version,
     hga_workspace_bytes,

@@ -68,6 +68,7 @@ def load_library():
     lib.hga_rope.argtypes = [P, V, I, V, F, V]
     lib.hga_build_summaries.argtypes = [P, V, V, F, F, V]
     lib.hga_route.argtypes = [P, F, F, F, V, F, V, V, F, V, V, C.c_size_t, V]
+    lib.hga_route_static.argtypes = [P, F, F, F, V, F, V, V, F, V, V]
     lib.hga_route_max.argtypes = [P, V, F, F, V, F, V, V, F, V, V, C.c_size_t, V]
     lib.hga_attend.argtypes = [P, V, V, V, V, V, F, V]
     lib.hga_prefill.argtypes = [P, C.POINTER(_CBuffers), V]
@@ -216,7 +217,33 @@ class RouteResult:
     group_idx: torch.Tensor
     group_score: torch.Tensor
     n_groups: torch.Tensor
-    workspace: torch.Tensor  # the chunk-score matrix [B, Hkv, n_b, n_b] lives here (lower triangle valid)
+    workspace: Optional[torch.Tensor]  # the chunk-score matrix [B, Hkv, n_b, n_b] lives here (lower triangle valid)
+
+
+ROUTE_STATIC_MAX_BYTES = 16 << 20  # HGA_ROUTE_STATIC_MAX_BYTES
+
+
+def hga_route_static(p: Params, q_pooled: torch.Tensor, chunk_sum: torch.Tensor, group_sum: torch.Tensor,
+                     out: Optional["RouteResult"] = None) -> "RouteResult":
+    """S2 + S3 with the library's static device scratch: no workspace argument, no allocation inside the C call.  Pass `out`
+    (a RouteResult from an earlier call) to make the Python side allocation-free too."""
+    dev = q_pooled.device
+    units = (p.batch, p.n_kv_heads, p.n_blocks)
+    r = out
+    if r is None:
+        r = RouteResult(
+            chunk_idx=torch.empty(units + (max(p.topk_chunks, 1),), dtype=torch.int32, device=dev),
+            chunk_score=torch.empty(units + (max(p.topk_chunks, 1),), dtype=torch.float32, device=dev),
+            n_chunks=torch.empty(units, dtype=torch.int32, device=dev),
+            group_idx=torch.empty(units + (max(p.topk_groups, 1),), dtype=torch.int32, device=dev),
+            group_score=torch.empty(units + (max(p.topk_groups, 1),), dtype=torch.float32, device=dev),
+            n_groups=torch.empty(units, dtype=torch.int32, device=dev),
+            workspace=None,
+        )
+    _check(load_library().hga_route_static(C.byref(p.c()), _ptr(q_pooled), _ptr(chunk_sum), _ptr(group_sum),
+                                           _ptr(r.chunk_idx), _ptr(r.chunk_score), _ptr(r.n_chunks), _ptr(r.group_idx),
+                                           _ptr(r.group_score), _ptr(r.n_groups), _stream()), "hga_route_static")
+    return r
 
 
 def hga_route(p: Params, q_pooled: torch.Tensor, chunk_sum: torch.Tensor, group_sum: torch.Tensor,

@@ -176,6 +176,20 @@ hga_status hga_route(const hga_params* p, const float* q_pooled, const float* ch
                       n_groups, (float*)workspace, (cudaStream_t)stream);
 }
 
+hga_status hga_route_static(const hga_params* p, const float* q_pooled, const float* chunk_sum, const float* group_sum,
+                            int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
+                            float* group_score, int32_t* n_groups, void* stream) {
+  Derived d;
+  hga_status st = derive(p, &d, nullptr);
+  if (st != HGA_OK) return st;
+  if (!q_pooled || !chunk_sum || !chunk_idx) return HGA_ERR_INVALID_ARG;
+  if (d.Kg > 0 && (!group_sum || !group_idx)) return HGA_ERR_INVALID_ARG;
+  if (!aligned16(q_pooled) || !aligned16(chunk_sum) || !aligned16(group_sum)) return HGA_ERR_INVALID_ARG;
+  if (d.route_max) return HGA_ERR_INVALID_ARG;  // per-query scores need q_rot: hga_route_max
+  return launch_route_static(d, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
+                             n_groups, (cudaStream_t)stream);
+}
+
 hga_status hga_route_max(const hga_params* p, const void* q_rot, const float* chunk_sum, const float* group_sum,
                          int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx, float* group_score,
                          int32_t* n_groups, void* workspace, size_t workspace_bytes, void* stream) {

@@ -101,6 +101,9 @@ hga_status launch_rope_summaries(const Derived& d, const RopeFreq& f, const void
 hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
                         int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s);
+hga_status launch_route_static(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
+                               int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
+                               float* group_score, int32_t* n_groups, cudaStream_t s);
 size_t route_max_ws_bytes(const Derived& d);
 hga_status launch_route_max(const Derived& d, const void* q_rot, const float* chunk_sum, const float* group_sum,
                             int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,

@@ -9,6 +9,7 @@
 //                  C/g_s groups of every kept chunk are scored (warp-cooperative fp64 dot products) and the top-K_g kept.
 #include <math_constants.h>
 
+#include <mutex>
 #include <type_traits>
 
 #include "hga_common.cuh"
@@ -1320,6 +1321,56 @@ hga_status launch_route_max(const Derived& d, const void* q_rot, const float* ch
                                          n_groups, n_units, d.jb, d.nj, d.n_b, d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap,
                                          per_warp, 2, gscores, nullptr);
   return launch_status();
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// hga_route_static: S2 + S3 for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that
+// forbid cudaMalloc) and have no workspace to pass.  The chunk-score matrix lives in a file-scope device array of
+// HGA_ROUTE_STATIC_MAX_BYTES (16 MiB: BASELINE.json configs[4], B 1 x H_kv 4 x 1024 x 1024 floats, fits exactly); every
+// GPU that loads the library holds it until the process exits.  In host code `g_route_static` is only the host-side
+// stand-in of the symbol, never a device address: the address comes from cudaGetSymbolAddress, once per device with that
+// device current.  No cudaMalloc / cudaFree / allocating library routine on this path.  All calls share the array, which
+// keeps the previous call's contents; nothing has to start at zero (score_kernel writes every entry the selection kernels
+// read, in the same call), but two calls that overlap on the GPU -- different streams, or graphs replayed concurrently --
+// race on it.
+// ----------------------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t kRouteStaticFloats = (size_t)HGA_ROUTE_STATIC_MAX_BYTES / sizeof(float);
+static __device__ __align__(256) float g_route_static[kRouteStaticFloats];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_route_static_mu;
+float* g_route_static_ptr[kMaxDevices] = {};  // device address of g_route_static on device i (nullptr: not looked up yet)
+
+// Device address of the scratch array on the current device; looked up once per device.
+hga_status route_static_scratch(float** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return HGA_ERR_CUDA;
+  std::lock_guard<std::mutex> lock(g_route_static_mu);
+  if (g_route_static_ptr[dev] == nullptr) {
+    float* ptr = nullptr;
+    if (cudaGetSymbolAddress((void**)&ptr, g_route_static) != cudaSuccess || ptr == nullptr) {
+      cudaGetLastError();  // leave no sticky-looking error behind for the caller's own checks
+      return HGA_ERR_CUDA;
+    }
+    g_route_static_ptr[dev] = ptr;
+  }
+  *out = g_route_static_ptr[dev];
+  return HGA_OK;
+}
+}  // namespace
+
+hga_status launch_route_static(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
+                               int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
+                               float* group_score, int32_t* n_groups, cudaStream_t s) {
+  // the same [B, Hkv, n_b, n_b] matrix hga_route asks its caller for; larger problems are refused, never truncated
+  const size_t need = (size_t)d.B * d.Hkv * d.n_b * d.n_b;
+  if (need > kRouteStaticFloats) return HGA_ERR_WORKSPACE;
+  float* scratch = nullptr;
+  hga_status st = route_static_scratch(&scratch);
+  if (st != HGA_OK) return st;
+  return launch_route(d, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score, n_groups,
+                      scratch, s);
 }
 
 }  // namespace hga
