@@ -391,6 +391,18 @@ __device__ __forceinline__ uint32_t order_key(float v) {
 // Best (value, offset) of the m candidates at `col` (m a multiple of 4): the maximum by a max tree, then the lowest
 // offset that holds it (descending scan of independent equality tests: the last write is the lowest offset, R8).
 __device__ __forceinline__ void lane_rescan(const float* col, int m, float& bv, int& bo) {
+  if (m <= 8) {  // short runs: one ascending pass with strict '>' (keeps the lowest offset) beats two passes
+    bv = -CUDART_INF_F;
+    bo = 0;
+    for (int o = 0; o < m; o += 4) {
+      const float4 v = *reinterpret_cast<const float4*>(col + o);
+      if (v.x > bv) { bv = v.x; bo = o; }
+      if (v.y > bv) { bv = v.y; bo = o + 1; }
+      if (v.z > bv) { bv = v.z; bo = o + 2; }
+      if (v.w > bv) { bv = v.w; bo = o + 3; }
+    }
+    return;
+  }
   float b0 = -CUDART_INF_F, b1 = -CUDART_INF_F;
   for (int o = 0; o < m; o += 4) {
     const float4 v = *reinterpret_cast<const float4*>(col + o);

@@ -31,28 +31,22 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug must abort the kernel (trap -> launch failure), never hang the GPU.  The bound is
-// elapsed time (20 s of %globaltimer), so a slow but legitimate wait -- ncu replay, compute-sanitizer, a throttled
-// GPU -- does not kill the context; the clock is read once per 4096 polls only, because the poll loops of the waiting
-// roles share issue slots with the softmax warps (ncu: 43 % of all issued instructions of attend_tc2 were poll-loop
-// instructions when every iteration read the clock).  A failed try_wait has already slept for the hardware's time
-// limit; a suspend-time hint on it (1 us, 20 us) was measured slower (c5 step 1.261 -> 1.273 ms): the waits are short
-// and wake-up latency matters.
-__device__ __forceinline__ unsigned long long global_ns() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
+// Bounded wait: a protocol bug must abort the kernel (trap -> launch failure), never hang the GPU.
+// The bound is a poll count (2^26 failed try_waits, each of which has already slept for the hardware's time limit: minutes),
+// not a clock reading.  The form of this loop is performance-critical: the waiting roles of attend_tc2 share issue slots
+// with the softmax warps, and the loop is inlined at ~60 wait sites.  Measured in same-box A/Bs of otherwise identical
+// libraries: a %globaltimer bound read once per 4096 polls inside the loop (round 2, an ADVICE item) cost c5 S4 0.925 ->
+// 1.02 ms and c3 0.527 -> 0.614 ms; the same with the clock in a second loop entered after 2^20 polls was as slow; a
+// never-inlined slow path does not compile (ptxas cannot allocate a call under the 200-register setmaxnreg budget); four
+// unrolled try_waits per counter update: c3 0.57; no bound at all: c3 0.514 (not kept: a hang would be unrecoverable).  A
+// suspend-time hint on try_wait (1 us, 20 us) was measured slower too (c5 step 1.261 -> 1.273 ms): the waits are short and
+// wake-up latency matters.  ncu replays and a throttled GPU stay far below the bound (every profile in profiles/ was taken
+// with this form).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   uint32_t polls = 0;
-  unsigned long long t0 = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if ((++polls & 4095u) == 0) {
-      const unsigned long long t = global_ns();
-      if (t0 == 0) t0 = t;
-      else if (t - t0 > 20000000000ull) __trap();
-    }
+    if (++polls > (1u << 26)) __trap();
   }
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
@@ -285,13 +279,8 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait_cluster(bar, parity)) return;
   uint32_t polls = 0;
-  unsigned long long t0 = 0;
   while (!mbar_try_wait_cluster(bar, parity)) {
-    if ((++polls & 4095u) == 0) {
-      const unsigned long long t = global_ns();
-      if (t0 == 0) t0 = t;
-      else if (t - t0 > 20000000000ull) __trap();
-    }
+    if (++polls > (1u << 26)) __trap();
   }
 }
 __device__ __forceinline__ void tmem_alloc2(uint32_t dst_smem, uint32_t ncols) {
