@@ -40,11 +40,23 @@ __device__ unsigned long long g_rt[32];
 constexpr int kTile = 64;
 constexpr int kSlab = 32;
 
-// 64 x 64 score tile per 64-thread CTA, 8 x 8 accumulators per thread: per k-step a thread reads 8 + 8 doubles for
-// 64 DFMAs, which balances the shared-memory pipe against the fp64 pipe (a 4 x 4 micro-tile is LDS-bound 2:1).
-// Thread (tx, ty) owns rows 16a + 2ty + {0,1} and columns 16b + 2tx + {0,1} (a, b = 0..3): every LDS.128 of a
-// quarter-warp covers 128 contiguous bytes (S) or one broadcast address (Q).
-__global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_pooled, const float* __restrict__ chunk_sum,
+// 64 x 64 score tile per 128-thread CTA on the fp64 tensor-core instruction (mma.sync.m8n8k4.f64): warp (wr, wc) owns the
+// 32 x 32 quadrant, i.e. 4 x 4 fragments of 8 x 8, 32 accumulator doubles per thread.  DMMA runs at the DFMA rate (64 FMA per
+// clock and SM, csrc/microbench/fp64_throughput.cu) but takes its operands once per warp: a k = 4 step costs a thread 8 doubles
+// from shared memory for 128 FMAs, where the DFMA micro-tiles cost 12 (4 x 8 tile) or 16 (8 x 8) doubles for 32 / 64 -- and
+// the register-file return path of shared memory (128 B per clock and SM) was what bound those forms (ncu: 5.6 M wavefronts
+// against 4.5 M cycles of fp64 work, fp64 pipe 45 % active).  Products and sums are fp64 as before; the order of the four
+// products inside one instruction is the hardware's (the result is compared with the oracle at 1e-6 relative, R15).
+// Shared layout [k][row] with a row pitch of 72 doubles: the four k-rows of a fragment fall into two disjoint bank halves.
+constexpr int kPitch = kTile + 8;
+
+__device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(128) score_kernel(const float* __restrict__ q_pooled, const float* __restrict__ chunk_sum,
                                                    float* __restrict__ scores, int n_b, int D, int F, int L_eff, int jb, int je) {
   // triangular tile index -> (tj, tc), tc <= tj
   const int ti = blockIdx.x;
@@ -64,61 +76,67 @@ __global__ void __launch_bounds__(64) score_kernel(const float* __restrict__ q_p
   const float* S = chunk_sum + slice * (size_t)n_b * D;
   float* out = scores + slice * (size_t)n_b * n_b;
 
-  __shared__ __align__(16) double Qs[kSlab][kTile];
-  __shared__ __align__(16) double Ss[kSlab][kTile];
-  const int tid = threadIdx.x, tx = tid % 8, ty = tid / 8;
-  double acc[8][8];
+  __shared__ __align__(16) double Qs[kSlab][kPitch];
+  __shared__ __align__(16) double Ss[kSlab][kPitch];
+  const int tid = threadIdx.x, lane = tid % 32, warp = tid / 32;
+  const int wr = (warp / 2) * 32, wc = (warp % 2) * 32;  // this warp's quadrant of the tile
+  const int fr = lane / 4, fk = lane % 4;                // fragment coordinates of this lane
+  double acc[4][4][2];
 #pragma unroll
-  for (int a = 0; a < 8; ++a)
+  for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int b = 0; b < 8; ++b) acc[a][b] = 0.0;
+    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
+  // threads 0..63 stage row tid of Q, threads 64..127 row tid - 64 of S: 32 consecutive floats per slab, converted once; the
+  // next slab's floats are fetched into registers before the current slab is consumed
+  const int rr = tid & 63;
+  const bool is_q = tid < 64;
+  const int srow = (is_q ? j0 : c0) + rr;
+  const bool ok = srow < n_b;
+  const float4* src = reinterpret_cast<const float4*>((is_q ? Q : S) + (size_t)srow * D);
+  double(*dst)[kPitch] = is_q ? Qs : Ss;
+  float4 pre[kSlab / 4];
+#pragma unroll
+  for (int v4 = 0; v4 < kSlab / 4; ++v4) pre[v4] = ok ? src[v4] : make_float4(0.f, 0.f, 0.f, 0.f);
   for (int k0 = 0; k0 < D; k0 += kSlab) {
     __syncthreads();  // previous slab fully consumed
-    {
-      // thread `tid` stages row tid of both operands: 32 consecutive floats each, converted once to double
-      const bool qok = j0 + tid < n_b, sok = c0 + tid < n_b;
-      const float4* qp = reinterpret_cast<const float4*>(Q + (size_t)(j0 + tid) * D + k0);
-      const float4* sp = reinterpret_cast<const float4*>(S + (size_t)(c0 + tid) * D + k0);
 #pragma unroll
-      for (int v4 = 0; v4 < kSlab / 4; ++v4) {
-        const float4 qv = qok ? qp[v4] : make_float4(0.f, 0.f, 0.f, 0.f);
-        const float4 sv = sok ? sp[v4] : make_float4(0.f, 0.f, 0.f, 0.f);
-        Qs[v4 * 4 + 0][tid] = (double)qv.x; Qs[v4 * 4 + 1][tid] = (double)qv.y;
-        Qs[v4 * 4 + 2][tid] = (double)qv.z; Qs[v4 * 4 + 3][tid] = (double)qv.w;
-        Ss[v4 * 4 + 0][tid] = (double)sv.x; Ss[v4 * 4 + 1][tid] = (double)sv.y;
-        Ss[v4 * 4 + 2][tid] = (double)sv.z; Ss[v4 * 4 + 3][tid] = (double)sv.w;
-      }
+    for (int v4 = 0; v4 < kSlab / 4; ++v4) {
+      dst[v4 * 4 + 0][rr] = (double)pre[v4].x; dst[v4 * 4 + 1][rr] = (double)pre[v4].y;
+      dst[v4 * 4 + 2][rr] = (double)pre[v4].z; dst[v4 * 4 + 3][rr] = (double)pre[v4].w;
+    }
+    if (k0 + kSlab < D) {
+#pragma unroll
+      for (int v4 = 0; v4 < kSlab / 4; ++v4) pre[v4] = ok ? src[(k0 + kSlab) / 4 + v4] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
     __syncthreads();
-#pragma unroll 4
-    for (int k = 0; k < kSlab; ++k) {
-      double qa[8], sb[8];
+#pragma unroll 2
+    for (int k = 0; k < kSlab; k += 4) {  // d ascending in steps of four
+      double a[4], b[4];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
-        const double2 qv = *reinterpret_cast<const double2*>(&Qs[k][16 * i + 2 * ty]);
-        const double2 sv = *reinterpret_cast<const double2*>(&Ss[k][16 * i + 2 * tx]);
-        qa[2 * i] = qv.x; qa[2 * i + 1] = qv.y;
-        sb[2 * i] = sv.x; sb[2 * i + 1] = sv.y;
+        a[i] = Qs[k + fk][wr + 8 * i + fr];  // A[row][k]: row = lane / 4, k = lane % 4
+        b[i] = Ss[k + fk][wc + 8 * i + fr];  // B[k][col]: k = lane % 4, col = lane / 4
       }
 #pragma unroll
-      for (int a = 0; a < 8; ++a)
+      for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int b = 0; b < 8; ++b) acc[a][b] = fma(qa[a], sb[b], acc[a][b]);  // d ascending: fixed order
+        for (int j = 0; j < 4; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
     }
   }
+  // C fragment: row = lane / 4, columns 2 (lane % 4) + {0, 1}
 #pragma unroll
-  for (int a = 0; a < 8; ++a) {
-    const int j = j0 + 16 * (a / 2) + 2 * ty + (a % 2);
+  for (int i = 0; i < 4; ++i) {
+    const int j = j0 + wr + 8 * i + fr;
     if (j >= je || j < jb) continue;
 #pragma unroll
-    for (int b2 = 0; b2 < 4; ++b2) {
-      const int c = c0 + 16 * b2 + 2 * tx;
+    for (int jj = 0; jj < 4; ++jj) {
+      const int c = c0 + wc + 8 * jj + 2 * fk;
       if (c + 1 < n_b && (n_b % 2) == 0) {
-        *reinterpret_cast<float2*>(out + (size_t)j * n_b + c) = make_float2((float)acc[a][2 * b2], (float)acc[a][2 * b2 + 1]);
+        *reinterpret_cast<float2*>(out + (size_t)j * n_b + c) = make_float2((float)acc[i][jj][0], (float)acc[i][jj][1]);
       } else {
-        if (c < n_b) out[(size_t)j * n_b + c] = (float)acc[a][2 * b2];
-        if (c + 1 < n_b) out[(size_t)j * n_b + c + 1] = (float)acc[a][2 * b2 + 1];
+        if (c < n_b) out[(size_t)j * n_b + c] = (float)acc[i][jj][0];
+        if (c + 1 < n_b) out[(size_t)j * n_b + c + 1] = (float)acc[i][jj][1];
       }
     }
   }
@@ -617,7 +635,7 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
                         float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
   const int nt = (d.n_b + kTile - 1) / kTile;
   dim3 grid(nt * (nt + 1) / 2, d.Hkv, d.B);
-  score_kernel<<<grid, 64, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff, d.jb, d.jb + d.nj);
+  score_kernel<<<grid, 128, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff, d.jb, d.jb + d.nj);
   if (cudaGetLastError() != cudaSuccess) return HGA_ERR_CUDA;
 
   const int n_units = d.B * d.Hkv * d.nj;

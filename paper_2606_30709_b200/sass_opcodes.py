@@ -12,7 +12,7 @@ import sys
 
 from .binding import lib_path
 
-OPS = ["UTCHMMA", "UTCBAR", "LDTM", "STTM", "UTMALDG", "UTMASTG", "UBLKCP", "SYNCS", "MUFU.EX2", "DFMA", "CREDUX", "HMMA"]
+OPS = ["UTCHMMA", "UTCBAR", "LDTM", "STTM", "UTMALDG", "UTMASTG", "UBLKCP", "SYNCS", "MUFU.EX2", "DFMA", "DMMA", "CREDUX", "HMMA"]
 
 
 def kernel_opcodes(so: str):
