@@ -438,8 +438,27 @@ __device__ __forceinline__ void lane_rescan(const float* col, int m, float& bv, 
   }
 }
 
-template <int D>
-__global__ void __launch_bounds__(128) select_fast_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
+// Register-resident form of lane_rescan for a lane that keeps its M candidates in registers (static indexing only).
+template <int M>
+__device__ __forceinline__ void reg_rescan(const float (&v)[M], float& bv, int& bo) {
+  float b0 = -CUDART_INF_F, b1 = -CUDART_INF_F;
+#pragma unroll
+  for (int o = 0; o < M; o += 4) {
+    b0 = tc::max3(b0, v[o], v[o + 1]);
+    b1 = tc::max3(b1, v[o + 2], v[o + 3]);
+  }
+  bv = fmaxf(b0, b1);
+  bo = 0;
+#pragma unroll
+  for (int o = M - 1; o >= 0; --o)
+    if (v[o] == bv) bo = o;  // the last write is the lowest offset (R8)
+}
+
+// M > 0: every lane keeps its run of M = 2^lm candidates in registers during the top-K_c rounds (the owner of a round's
+// winner removes it and rescans without touching shared memory: c5 route 73 -> 69 us, c4 46 -> 44 us); M == 0: the run
+// lives in shared memory (any lm; runs of 8 and shorter measured no gain in registers).
+template <int D, int M>
+__global__ void __launch_bounds__(128, 7) select_fast_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
                                                           const float* __restrict__ group_sum, int32_t* __restrict__ chunk_idx,
                                                           float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
                                                           int32_t* __restrict__ group_idx, float* __restrict__ group_score,
@@ -482,7 +501,18 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
   float* col = work + lane * stride;
   float bv = -CUDART_INF_F;
   int bo = 0;
-  if (lane < n_lanes) lane_rescan(col, m, bv, bo);
+  float v[M > 0 ? M : 1];
+  if constexpr (M > 0) {
+#pragma unroll
+    for (int o = 0; o < M; o += 4) {
+      const float4 t = lane < n_lanes ? *reinterpret_cast<const float4*>(col + o)
+                                      : make_float4(-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F);
+      v[o] = t.x; v[o + 1] = t.y; v[o + 2] = t.z; v[o + 3] = t.w;
+    }
+    reg_rescan<M>(v, bv, bo);
+  } else {
+    if (lane < n_lanes) lane_rescan(col, m, bv, bo);
+  }
   HGA_RT(16);
 
   // ---- top-K_c: one winner per round, kept in lane r ---------------------------------------------------------
@@ -506,8 +536,15 @@ __global__ void __launch_bounds__(128) select_fast_kernel(const float* __restric
         wsc = vstar;
       }
       if (lane == owner) {
-        col[bo] = -CUDART_INF_F;
-        lane_rescan(col, m, bv, bo);
+        if constexpr (M > 0) {
+#pragma unroll
+          for (int o = 0; o < M; ++o)
+            if (o == bo) v[o] = -CUDART_INF_F;
+          reg_rescan<M>(v, bv, bo);
+        } else {
+          col[bo] = -CUDART_INF_F;
+          lane_rescan(col, m, bv, bo);
+        }
       }
     }
   }
@@ -650,7 +687,15 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
     while (warps > 1 && (size_t)warps * per_warp_bytes > 200 * 1024) warps >>= 1;
     const size_t smem = (size_t)warps * per_warp_bytes;
     if (smem <= 200 * 1024) {
-      auto kern = d.D == 128 ? select_fast_kernel<128> : select_fast_kernel<64>;
+      auto pick = [&](auto Dc) {
+        constexpr int DD = decltype(Dc)::value;
+        switch (lm) {
+          case 4: return select_fast_kernel<DD, 16>;
+          case 5: return select_fast_kernel<DD, 32>;
+          default: return select_fast_kernel<DD, 0>;
+        }
+      };
+      auto kern = d.D == 128 ? pick(std::integral_constant<int, 128>{}) : pick(std::integral_constant<int, 64>{});
       HGA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       kern<<<(n_units + warps - 1) / warps, warps * 32, smem, s>>>(score_ws, q_pooled, group_sum, chunk_idx, chunk_score,
                                                                    n_chunks, group_idx, group_score, n_groups, n_units,
