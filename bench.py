@@ -514,6 +514,24 @@ def run_ours(args, w):
                                              "storing them, S4 reads q_raw and applies RoPE to its query tiles in shared memory; "
                                              "compare with stages.* of the default path -- built, parity-green and slower")
             del buf_f
+            # S2 + S3 called alone, with and without the optional score outputs (chunk_score / group_score may be NULL, hga.h).
+            # At c4 / c5 K_g = 4 K_c keeps every group of the kept chunks, so without group_score the group stage has nothing
+            # to compute.  The timed steps above always pass the score outputs (the parity tests compare them).
+            wsr = torch.empty(hga.hga_workspace_bytes(p), dtype=torch.uint8, device="cuda")
+            cpr = p.c()
+
+            def route_alone(with_scores):
+                def f():
+                    rc = lib.hga_route(C.byref(cpr), buf.q_pooled.data_ptr(), buf.chunk_sum.data_ptr(), buf.group_sum.data_ptr(),
+                                       buf.chunk_idx.data_ptr(), buf.chunk_score.data_ptr() if with_scores else None,
+                                       buf.n_chunks.data_ptr(), buf.group_idx.data_ptr(),
+                                       buf.group_score.data_ptr() if with_scores else None, buf.n_groups.data_ptr(),
+                                       wsr.data_ptr(), wsr.numel(), torch.cuda.current_stream().cuda_stream)
+                    assert rc == 0
+                return sep(f, reps=20)
+
+            variants["route_alone_ms"] = {"with_score_outputs": route_alone(True), "without_score_outputs": route_alone(False)}
+            del wsr
         except Exception as e:  # a variant must never sink the headline line
             variants = {"error": str(e)}
 

@@ -536,6 +536,25 @@ def test_fused_q_rope_c5_whole_slice_and_rejections():
         hga.hga_prefill(p.replace(flags=2), dq, dk, dv)
 
 
+@pytest.mark.parametrize("name", ["c4", "c2"])
+def test_route_without_score_outputs_gives_the_same_lists(name):
+    """chunk_score / group_score / n_chunks / n_groups are optional outputs (hga.h).  Without group_score, and with K_g keeping
+    every group of the kept chunks (c4: K_g = 4 K_c), select_fast_kernel skips the group scoring altogether; the lists must
+    not change.  c2 (K_g < 4 K_c) still scores."""
+    import ctypes as C
+    w = W.get(name)
+    q, k, v = W.generate(w, 0)
+    p, buf = parity.run_gpu(w, q, k, v)
+    lib, cp = hga.load_library(), p.c()
+    ci, gi = torch.full_like(buf.chunk_idx, -7), torch.full_like(buf.group_idx, -7)
+    rc = lib.hga_route(C.byref(cp), buf.q_pooled.data_ptr(), buf.chunk_sum.data_ptr(), buf.group_sum.data_ptr(), ci.data_ptr(),
+                       None, None, gi.data_ptr(), None, None, buf.workspace.data_ptr(), buf.workspace.numel(),
+                       torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert rc == 0
+    assert torch.equal(ci, buf.chunk_idx) and torch.equal(gi, buf.group_idx)
+
+
 def test_route_max_mode_c5_full_size_sampled():
     """The max rule at BASELINE.json configs[4] (64K, Qwen3 head shape): sampled blocks of two slices against the oracle."""
     w = dataclasses.replace(W.get("c5"), route_max=True)
