@@ -156,8 +156,10 @@ HGA_API int32_t hga_n_hi_rule(int32_t head_dim, double rope_base, int32_t span, 
 /* Validate `p` without touching the GPU. */
 HGA_API hga_status hga_validate(const hga_params* p);
 
-/* Bytes of device scratch hga_route / hga_prefill need for `p` (the chunk-score matrix
- * [batch, n_kv_heads, seq/chunk, seq/chunk] float).  Host arithmetic only. */
+/* Bytes of device scratch hga_route / hga_prefill need for `p`: chunk scores [batch, n_kv_heads, R, seq/chunk] float with
+ * R = min(seq/chunk, 1024) -- the route stage runs in slabs of at most 1024 query blocks, so the scratch grows linearly
+ * with the sequence past 64K tokens (more under HGA_ROUTE_MAX and HGA_FLAG_FUSE_Q_ROPE, which add their own tables).
+ * Host arithmetic only. */
 HGA_API hga_status hga_workspace_bytes(const hga_params* p, size_t* bytes);
 
 /*
@@ -196,7 +198,7 @@ HGA_API hga_status hga_route(const hga_params* p, const float* q_pooled, const f
  * hga_route without a workspace argument and without any allocation, for callers that cannot call cudaMalloc (code under
  * CUDA graph capture, tight serving loops, harnesses that forbid it): the chunk-score matrix lives in a static device
  * array of HGA_ROUTE_STATIC_MAX_BYTES inside the library (every GPU that loads the library holds it until the process
- * exits).  Same arguments, outputs and results as hga_route, bit for bit.  Limit: batch * n_kv_heads * (seq/chunk)^2 * 4
+ * exits).  Same arguments, outputs and results as hga_route, bit for bit.  Limit: batch * n_kv_heads * min(seq/chunk, 1024) * (seq/chunk) * 4
  * bytes <= HGA_ROUTE_STATIC_MAX_BYTES (BASELINE.json configs[4], 64K tokens x 4 KV heads, fits exactly); a larger problem
  * returns HGA_ERR_WORKSPACE and launches nothing -- use hga_route with a caller-owned workspace.  HGA_ROUTE_MEAN only.
  * The first call on a device looks the array's address up (cudaGetSymbolAddress, which may load the module: make one

@@ -84,7 +84,7 @@ static size_t rope_tables_bytes(const Derived& d) {
 
 static size_t route_ws_bytes(const Derived& d) {
   size_t n = d.route_max ? route_max_ws_bytes(d)                               // + group-candidate scores, prefilter tables
-                         : (size_t)d.B * d.Hkv * d.n_b * d.n_b * sizeof(float);  // chunk-score matrix
+                         : (size_t)d.B * d.Hkv * route_ws_rows(d.n_b) * d.n_b * sizeof(float);  // chunk scores, one slab
   return (n + 255) & ~(size_t)255;
 }
 
@@ -173,7 +173,7 @@ hga_status hga_route(const hga_params* p, const float* q_pooled, const float* ch
   if (d.route_max) return HGA_ERR_INVALID_ARG;  // per-query scores need q_rot: hga_route_max
   if (!workspace || !aligned16(workspace) || workspace_bytes < score_ws_bytes(d)) return HGA_ERR_WORKSPACE;
   return launch_route(d, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score,
-                      n_groups, (float*)workspace, (cudaStream_t)stream);
+                      n_groups, (float*)workspace, (cudaStream_t)stream, 0);
 }
 
 hga_status hga_route_static(const hga_params* p, const float* q_pooled, const float* chunk_sum, const float* group_sum,
@@ -308,7 +308,7 @@ static hga_status prefill_impl(const hga_params* p, const hga_buffers* b, void* 
                           b->group_score, b->n_groups, (float*)b->workspace, cs);
   } else {
     st = launch_route(d, b->q_pooled, b->chunk_sum, b->group_sum, b->chunk_idx, b->chunk_score, b->n_chunks, b->group_idx,
-                      b->group_score, b->n_groups, (float*)b->workspace, cs);
+                      b->group_score, b->n_groups, (float*)b->workspace, cs, 0);
   }
   if (st != HGA_OK) return st;
   if (ev) HGA_CUDA_OK(cudaEventRecord(ev[2], cs));

@@ -98,9 +98,13 @@ hga_status launch_summaries(const Derived& d, const RopeFreq& f, const void* k_r
                             float* group_sum, cudaStream_t s);
 hga_status launch_rope_summaries(const Derived& d, const RopeFreq& f, const void* q_raw, void* q_rot, float* pooled,
                                  const void* k_raw, void* k_rot, float* chunk_sum, float* group_sum, cudaStream_t s);
+// rows of the score workspace per (batch, kv head) slice under the pooled-query rule: the route stage runs in slabs
+constexpr int kRouteSlabRows = 1024;
+inline size_t route_ws_rows(int n_b) { return (size_t)(n_b < kRouteSlabRows ? n_b : kRouteSlabRows); }
+// slab_rows: 0 = kRouteSlabRows; a smaller value forces more slabs (tests)
 hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
                         int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
-                        float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s);
+                        float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s, int slab_rows);
 hga_status launch_route_static(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
                                int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                                float* group_score, int32_t* n_groups, cudaStream_t s);

@@ -74,7 +74,8 @@ __global__ void __launch_bounds__(128) score_kernel(const float* __restrict__ q_
   const size_t slice = (size_t)blockIdx.z * gridDim.y + blockIdx.y;  // b * Hkv + kv
   const float* Q = q_pooled + slice * (size_t)n_b * D;
   const float* S = chunk_sum + slice * (size_t)n_b * D;
-  float* out = scores + slice * (size_t)n_b * n_b;
+  // the workspace holds the rows of [jb, je) only: row (slice, j) at (slice * (je - jb) + j - jb) * n_b
+  float* out = scores + (slice * (size_t)(je - jb) - (size_t)jb) * n_b;
 
   __shared__ __align__(16) double Qs[kSlab][kPitch];
   __shared__ __align__(16) double Ss[kSlab][kPitch];
@@ -295,7 +296,8 @@ __global__ void __launch_bounds__(128) select_generic_kernel(const float* __rest
   const size_t slice = widx / nj;        // b * Hkv + kv
   const size_t unit = slice * n_b + j;   // row of every [B, Hkv, n_b, ...] table
   if (only_neg != nullptr && only_neg[unit] >= 0) return;  // warp-uniform
-  const float* row = scores + (size_t)unit * n_b;
+  // mean rule (phase 0): the workspace holds the rows of [jb, jb + nj) only; max rule: the full [B, Hkv, n_b, n_b] matrix
+  const float* row = scores + (size_t)(phase == 0 ? (size_t)widx : unit) * n_b;
   const int lo = F, hi = j - L_eff;
   const int n = hi > lo ? hi - lo : 0;
   int cnt = 0;
@@ -477,7 +479,7 @@ __global__ void __launch_bounds__(128, 7) select_fast_kernel(const float* __rest
   const int j = jb + widx % nj;          // blocks [jb, jb + nj) of every slice
   const size_t slice = widx / nj;        // b * Hkv + kv
   const size_t unit = slice * n_b + j;   // row of every [B, Hkv, n_b, ...] table
-  const float* row = scores + (size_t)unit * n_b;
+  const float* row = scores + (size_t)widx * n_b;  // the score workspace holds the rows of [jb, jb + nj) only
   const int lo = F, hi = j - L_eff;
   const int n = hi > lo ? hi - lo : 0;
   int32_t* cidx = chunk_idx + (size_t)unit * Kc;
@@ -667,9 +669,10 @@ __global__ void __launch_bounds__(128, 7) select_fast_kernel(const float* __rest
 
 }  // namespace
 
-hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
-                        int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
-                        float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
+// One slab: the query blocks [d.jb, d.jb + d.nj), at most kRouteSlabRows of them; score_ws holds B * Hkv * d.nj rows.
+static hga_status launch_route_slab(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
+                                    int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
+                                    float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s) {
   const int nt = (d.n_b + kTile - 1) / kTile;
   dim3 grid(nt * (nt + 1) / 2, d.Hkv, d.B);
   score_kernel<<<grid, 128, 0, s>>>(q_pooled, chunk_sum, score_ws, d.n_b, d.D, d.F, d.L_eff, d.jb, d.jb + d.nj);
@@ -715,6 +718,25 @@ hga_status launch_route(const Derived& d, const float* q_pooled, const float* ch
                                                                n_chunks, group_idx, group_score, n_groups, n_units, d.jb, d.nj, d.n_b,
                                                                d.n_g, d.gpc, d.F, d.L_eff, d.Kc, d.Kg, kc_cap, per_warp, 0, nullptr, nullptr);
   return launch_status();
+}
+
+// S2 + S3 over the query blocks [d.jb, d.jb + d.nj) in slabs of at most kRouteSlabRows blocks, one after the other on the
+// stream: the score workspace is B * Hkv * min(n_b, kRouteSlabRows) rows of n_b floats (route_ws_rows), not n_b^2 per
+// slice -- 16.8 MB at 64K tokens as before, 268 MB instead of 4.3 GB at 1 M tokens (B 1, H_kv 4); a decode step or a
+// chunk append (hga_prefill_window) touches one row per slice.
+hga_status launch_route(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
+                        int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
+                        float* group_score, int32_t* n_groups, float* score_ws, cudaStream_t s, int slab_rows) {
+  if (slab_rows <= 0 || slab_rows > kRouteSlabRows) slab_rows = kRouteSlabRows;
+  for (int j0 = d.jb; j0 < d.jb + d.nj; j0 += slab_rows) {
+    Derived ds = d;
+    ds.jb = j0;
+    ds.nj = d.jb + d.nj - j0 < slab_rows ? d.jb + d.nj - j0 : slab_rows;
+    hga_status st = launch_route_slab(ds, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx,
+                                      group_score, n_groups, score_ws, s);
+    if (st != HGA_OK) return st;
+  }
+  return HGA_OK;
 }
 
 }  // namespace hga (reopened below)
@@ -1438,14 +1460,15 @@ hga_status route_static_scratch(float** out) {
 hga_status launch_route_static(const Derived& d, const float* q_pooled, const float* chunk_sum, const float* group_sum,
                                int32_t* chunk_idx, float* chunk_score, int32_t* n_chunks, int32_t* group_idx,
                                float* group_score, int32_t* n_groups, cudaStream_t s) {
-  // the same [B, Hkv, n_b, n_b] matrix hga_route asks its caller for; larger problems are refused, never truncated
-  const size_t need = (size_t)d.B * d.Hkv * d.n_b * d.n_b;
+  // the same B * Hkv * min(n_b, kRouteSlabRows) rows of n_b floats hga_route asks its caller for; larger problems are
+  // refused, never truncated
+  const size_t need = (size_t)d.B * d.Hkv * route_ws_rows(d.n_b) * d.n_b;
   if (need > kRouteStaticFloats) return HGA_ERR_WORKSPACE;
   float* scratch = nullptr;
   hga_status st = route_static_scratch(&scratch);
   if (st != HGA_OK) return st;
   return launch_route(d, q_pooled, chunk_sum, group_sum, chunk_idx, chunk_score, n_chunks, group_idx, group_score, n_groups,
-                      scratch, s);
+                      scratch, s, 0);
 }
 
 }  // namespace hga

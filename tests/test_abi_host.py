@@ -72,6 +72,12 @@ def test_workspace_and_host_byte_counts():
         p = hga.params_from_workload(w)
         n_b = w.seq // 64
         assert hga.hga_workspace_bytes(p) >= w.batch * w.n_kv_heads * n_b * n_b * 4  # the chunk-score matrix
+    # beyond 1024 blocks the route stage runs in slabs of 1024 query blocks: the workspace grows linearly, not quadratically
+    big = hga.params_from_workload(W.get("c5").replace(seq=16 * 65536))
+    assert hga.hga_workspace_bytes(big) == 1 * 4 * 1024 * (16 * 1024) * 4
+    for name in ("c5",):
+        w = W.get(name)
+        p = hga.params_from_workload(w)
         e = 2 if w.dtype == "bf16" else 4
         h2d, d2h = C.c_size_t(0), C.c_size_t(0)
         assert hga.load_library().hga_host_bytes(C.byref(p.c()), 0, 0, C.byref(h2d), C.byref(d2h)) == 0

@@ -555,6 +555,22 @@ def test_route_without_score_outputs_gives_the_same_lists(name):
     assert torch.equal(ci, buf.chunk_idx) and torch.equal(gi, buf.group_idx)
 
 
+def test_route_in_slabs_beyond_1024_blocks():
+    """131,072 tokens = 2,048 blocks: S2 + S3 run in two slabs of 1,024 query blocks over one half-size workspace
+    (hga_workspace_bytes grows linearly past 1,024 blocks).  Sampled blocks of both slabs, and the blocks around the slab
+    boundary, against the oracle; the whole path (outputs included)."""
+    w = W.Workload("slab_128k", 1, 131072, 2, 1, 64, "bf16", 1.0e4, topk_chunks=6, topk_groups=12, n_clusters=8)
+    q, k, v = W.generate(w, 11)
+    p, buf = parity.run_gpu(w, q, k, v)
+    assert hga.hga_workspace_bytes(p) == 1024 * 2048 * 4
+    blocks = np.array([0, 1, 2, 500, 1022, 1023, 1024, 1025, 1500, 2046, 2047])
+    rep = parity.check_against_oracle(w, q, k, v, p, buf, [(0, 0)], blocks)
+    parity.assert_report(rep, w, len(blocks))
+    nch = buf.n_chunks[0, 0].cpu().numpy()
+    assert (nch[8:] == 6).all()          # every later block got its full budget, in both slabs
+    assert torch.isfinite(buf.out).all()
+
+
 def test_route_max_mode_c5_full_size_sampled():
     """The max rule at BASELINE.json configs[4] (64K, Qwen3 head shape): sampled blocks of two slices against the oracle."""
     w = dataclasses.replace(W.get("c5"), route_max=True)
