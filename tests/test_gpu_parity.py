@@ -555,6 +555,25 @@ def test_route_without_score_outputs_gives_the_same_lists(name):
     assert torch.equal(ci, buf.chunk_idx) and torch.equal(gi, buf.group_idx)
 
 
+def test_route_exact_ties_take_the_lowest_indices():
+    """Pooled-query rule with every chunk summary identical (keys periodic in the chunk length, RoPE positions wrapped at the
+    chunk length): all candidates of a block tie exactly -- also on the fp64 tensor-core instruction, which treats identical
+    columns identically -- and the lowest indices win (R8), in the register-resident top-K (16 candidates per lane at 512
+    blocks), the shared-memory form (8 per lane at 256 blocks) and the generic kernel (K_c > 32)."""
+    for n_blocks, Kc, Kg in ((512, 6, 12), (256, 6, 12), (256, 40, 50)):
+        w = W.Workload("ties_mean", 1, 64 * n_blocks, 4, 2, 64, "bf16", 1e4, topk_chunks=Kc, topk_groups=Kg, n_clusters=8,
+                       rope_pos_mod=64)
+        q, k, v = W.generate(w, 5)
+        k = np.ascontiguousarray(np.tile(k[:, :, :64], (1, 1, w.n_blocks, 1)))
+        p, buf = parity.run_gpu(w, q, k, v)
+        ci = buf.chunk_idx[0, 1].cpu().numpy()
+        assert list(ci[n_blocks - 1, :Kc]) == list(range(1, Kc + 1))   # F = 1: candidates start at chunk 1
+        assert list(ci[100, :Kc]) == list(range(1, Kc + 1))
+        blocks = _sample_blocks(w.n_blocks, 6, 2)
+        rep = parity.check_against_oracle(w, q, k, v, p, buf, [(0, 1)], blocks)
+        parity.assert_report(rep, w, len(blocks))
+
+
 def test_route_in_slabs_beyond_1024_blocks():
     """131,072 tokens = 2,048 blocks: S2 + S3 run in two slabs of 1,024 query blocks over one half-size workspace
     (hga_workspace_bytes grows linearly past 1,024 blocks).  Sampled blocks of both slabs, and the blocks around the slab
