@@ -54,11 +54,15 @@ def test_route_static_matches_hga_route_on_two_calls_in_a_row():
     assert torch.equal(got1.group_idx, b1.group_idx) and torch.equal(got2.group_idx, b2.group_idx)
     # the same call again into the same output tensors: identical, and the device's free memory does not move (no cudaMalloc
     # inside the call; the outputs are reused, so the Python side allocates nothing either)
-    free0 = torch.cuda.mem_get_info()[0]
-    again = hga.hga_route_static(p1, b1.q_pooled, b1.chunk_sum, b1.group_sum, out=got1)
-    again = hga.hga_route_static(p2, b2.q_pooled, b2.chunk_sum, b2.group_sum, out=got2)
-    torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free0
+    for attempt in range(3):  # mem_get_info is device-wide: tolerate an unrelated change once or twice, never a steady one
+        free0 = torch.cuda.mem_get_info()[0]
+        again = hga.hga_route_static(p1, b1.q_pooled, b1.chunk_sum, b1.group_sum, out=got1)
+        again = hga.hga_route_static(p2, b2.q_pooled, b2.chunk_sum, b2.group_sum, out=got2)
+        torch.cuda.synchronize()
+        if torch.cuda.mem_get_info()[0] == free0:
+            break
+    else:
+        raise AssertionError("device free memory moved across hga_route_static calls three times in a row")
     _assert_same(again, ref2, p2)
     _assert_same(got1, ref1, p1)
 
