@@ -460,7 +460,7 @@ __device__ __forceinline__ void reg_rescan(const float (&v)[M], float& bv, int& 
 // winner removes it and rescans without touching shared memory: c5 route 73 -> 69 us, c4 46 -> 44 us); M == 0: the run
 // lives in shared memory (any lm; runs of 8 and shorter measured no gain in registers).
 template <int D, int M>
-__global__ void __launch_bounds__(128, 7) select_fast_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
+__global__ void __launch_bounds__(128, (M > 0 ? 7 : 9)) select_fast_kernel(const float* __restrict__ scores, const float* __restrict__ q_pooled,
                                                           const float* __restrict__ group_sum, int32_t* __restrict__ chunk_idx,
                                                           float* __restrict__ chunk_score, int32_t* __restrict__ n_chunks,
                                                           int32_t* __restrict__ group_idx, float* __restrict__ group_score,
