@@ -617,6 +617,22 @@ __global__ void __launch_bounds__(128, (M > 0 ? 7 : 9)) select_fast_kernel(const
 #pragma unroll
     for (int i = 0; i < 4; ++i)
       if (lane + 32 * i < n_gc) taken |= 1u << i;
+  } else if (n_gc <= 64) {
+    // at most two candidates per lane: rank every candidate against all others (value descending, index ascending) with 64
+    // shuffles and keep the ranks below K_g -- one pass instead of K_g rounds of two warp reductions each
+    const uint32_t k0 = lane < n_gc ? order_key(gsc[0]) : 0u;          // 0 is below the key of any float, -inf included
+    const uint32_t k1 = lane + 32 < n_gc ? order_key(gsc[1]) : 0u;
+    int r0 = 0, r1 = 0;  // candidates that come before candidate lane / lane + 32
+#pragma unroll 8
+    for (int sl = 0; sl < 32; ++sl) {
+      const uint32_t a = __shfl_sync(kFull, k0, sl), b = __shfl_sync(kFull, k1, sl);  // candidates sl and sl + 32
+      r0 += (a > k0 || (a == k0 && sl < lane)) ? 1 : 0;
+      r0 += (b > k0) ? 1 : 0;                       // index sl + 32 > lane: a tie does not come before
+      r1 += (a >= k1) ? 1 : 0;                      // index sl < lane + 32: a tie comes before
+      r1 += (b > k1 || (b == k1 && sl < lane)) ? 1 : 0;
+    }
+    if (lane < n_gc && r0 < gtake) taken |= 1u;
+    if (lane + 32 < n_gc && r1 < gtake) taken |= 2u;
   } else {
     float wv[4];
 #pragma unroll
